@@ -1,0 +1,629 @@
+/*
+ * npfem_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64 CPU implementation of the npFEM nodal projective-FEM time step for closed
+ * triangular surface meshes (red blood cells, platelets).  It is the parity oracle for the CUDA
+ * library in paper_2011_04332_b200/ and shares no code with it.  Only tests/, bench.py's
+ * cpu_baseline / --impl reference legs and __graft_entry__.smoke() may load it.
+ *
+ * What it follows
+ * ---------------
+ *  - PAPER.md:56-60 (Introduction, eq. 2): elastodynamics, Newton's 2nd law per body.
+ *  - PAPER.md:66: "mass-lumped linear FE solver" on triangular surface meshes (:70), implicit.
+ *  - PAPER.md:90-95: derived from ShapeOp / projective dynamics [3], time stepping after Liu et
+ *    al. [11]; with no L-BFGS history and unit step length that scheme is the classic alternating
+ *    local/global sweep implemented here (reading A-1).
+ *  - PAPER.md:181: the body's potential energy is a sum of per-element energies, each with a weight
+ *    and parameters.
+ *  - BASELINE.json north_star: local step = projection of every triangle's strain, bending hinge
+ *    and area/volume constraint; global step = solve (M/h^2 + sum w A^T A) x = rhs.
+ * The paper prints none of the energies; every formula below is a READING listed in DESIGN.md
+ * (A-1 ... A-16).  Agreement with the real npFEM code is
+ * "parity unpinned"; what IS pinned (tests/test_oracle_pins.py) are invariants, closed forms,
+ * library routines and brute force.
+ *
+ * Formulation: ABSOLUTE positions, rhs b = M/h^2 s + sum w A^T p, dense Cholesky of A_sys.
+ * (The CUDA path uses a different algebra: cell-local coordinates and an increment form.)
+ * No blocking, no fusion, no reordering: one function per sentence of the algorithm.
+ * OpenMP is used over cells only (one cell per thread, as the paper's CPU branch maps one cell
+ * per core).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_OK 0
+#define ORACLE_EINVAL -1
+#define ORACLE_ENOMEM -2
+
+typedef struct {
+  double cell_mass;
+  double k_strain, s_min, s_max;
+  double k_area, a_min, a_max;
+  double k_bend;
+  double w_volume, v_min, v_max;
+  double c_alpha, c_beta;
+} oracle_material;
+
+typedef struct oracle_cell {
+  int n, T, H;
+  int32_t *tris;   /* [T][3] */
+  double *X;       /* rest positions [n][3] */
+  oracle_material mat;
+  double h;
+  double *G;       /* [T][2][3]: F^T = G [x_a; x_b; x_c] */
+  double *area;    /* [T] rest areas A_t */
+  double *mass;    /* [n] lumped masses */
+  int32_t *hinge;  /* [H][4] stencils (x0,x1,x2,x3) */
+  double *K;       /* [H][4] cotangent rows */
+  double *w_h;     /* [H] hinge weights */
+  double *r_h;     /* [H] rest magnitudes ||sum K_i X_i|| */
+  double V0;       /* rest volume */
+  double *A;       /* dense A_sys [n][n] */
+  double *L;       /* dense lower Cholesky factor of A_sys [n][n] */
+  double *LT;      /* its transpose, so that the backward substitution also reads rows */
+} oracle_cell;
+
+/* ---------------------------------------------------------------- small vector helpers */
+static void sub3(const double *a, const double *b, double *o) { o[0]=a[0]-b[0]; o[1]=a[1]-b[1]; o[2]=a[2]-b[2]; }
+static double dot3(const double *a, const double *b) { return a[0]*b[0]+a[1]*b[1]+a[2]*b[2]; }
+static void cross3(const double *a, const double *b, double *o) {
+  o[0]=a[1]*b[2]-a[2]*b[1]; o[1]=a[2]*b[0]-a[0]*b[2]; o[2]=a[0]*b[1]-a[1]*b[0];
+}
+static double norm3(const double *a) { return sqrt(dot3(a,a)); }
+static double clampd(double v, double lo, double hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+/* ---------------------------------------------------------------- geometry of the whole cell */
+/* V(x) = 1/6 sum_t x_a . (x_b x x_c)   (SURVEY.md 8(c) create step 4) */
+double oracle_volume(int T, const int32_t *tris, const double *x) {
+  double V = 0.0;
+  for (int t = 0; t < T; ++t) {
+    const double *a = x + 3*tris[3*t], *b = x + 3*tris[3*t+1], *c = x + 3*tris[3*t+2];
+    double bc[3]; cross3(b, c, bc);
+    V += dot3(a, bc);
+  }
+  return V / 6.0;
+}
+
+/* (grad V)_a += 1/6 x_b x x_c (cyclic) per triangle   (volume) */
+void oracle_volume_grad(int n, int T, const int32_t *tris, const double *x, double *g) {
+  memset(g, 0, sizeof(double) * 3 * (size_t)n);
+  for (int t = 0; t < T; ++t) {
+    int ia = tris[3*t], ib = tris[3*t+1], ic = tris[3*t+2];
+    const double *a = x + 3*ia, *b = x + 3*ib, *c = x + 3*ic;
+    double bc[3], ca[3], ab[3];
+    cross3(b, c, bc); cross3(c, a, ca); cross3(a, b, ab);
+    for (int k = 0; k < 3; ++k) {
+      g[3*ia+k] += bc[k] / 6.0;
+      g[3*ib+k] += ca[k] / 6.0;
+      g[3*ic+k] += ab[k] / 6.0;
+    }
+  }
+}
+
+/* ---------------------------------------------------------------- 3x2 thin SVD (one-sided Jacobi)
+ * F (row-major 3x2) = U diag(S) V^T with U 3x2 (row-major), S[0] >= S[1] >= 0, V 2x2 (row-major).
+ * For two columns one Hestenes rotation orthogonalises them exactly; it is repeated until the
+ * columns are orthogonal to rounding.  Pinned against LAPACK (numpy.linalg.svd) in the tests. */
+void oracle_svd32(const double *F, double *U, double *S, double *V) {
+  double a[3] = {F[0], F[2], F[4]}, b[3] = {F[1], F[3], F[5]};
+  double v00 = 1, v01 = 0, v10 = 0, v11 = 1;          /* V = I */
+  for (int sweep = 0; sweep < 30; ++sweep) {
+    double alpha = dot3(a,a), beta = dot3(b,b), gamma = dot3(a,b);
+    if (fabs(gamma) <= 1e-300 || fabs(gamma) <= 1e-17 * sqrt(alpha*beta)) break;
+    double zeta = (beta - alpha) / (2.0 * gamma);
+    double t = (zeta >= 0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta*zeta));
+    double c = 1.0 / sqrt(1.0 + t*t), s = c * t;
+    for (int k = 0; k < 3; ++k) {
+      double ak = a[k], bk = b[k];
+      a[k] = c*ak - s*bk;
+      b[k] = s*ak + c*bk;
+    }
+    double n00 = c*v00 - s*v01, n01 = s*v00 + c*v01;
+    double n10 = c*v10 - s*v11, n11 = s*v10 + c*v11;
+    v00 = n00; v01 = n01; v10 = n10; v11 = n11;
+  }
+  double s0 = norm3(a), s1 = norm3(b);
+  if (s1 > s0) {                                       /* sort descending: swap columns */
+    double tmp;
+    for (int k = 0; k < 3; ++k) { tmp = a[k]; a[k] = b[k]; b[k] = tmp; }
+    tmp = v00; v00 = v01; v01 = tmp;
+    tmp = v10; v10 = v11; v11 = tmp;
+    tmp = s0; s0 = s1; s1 = tmp;
+  }
+  double u0[3] = {0,0,0}, u1[3] = {0,0,0};
+  if (s0 > 0) { for (int k = 0; k < 3; ++k) u0[k] = a[k] / s0; } else { u0[0] = 1; }
+  if (s1 > 1e-300 && s1 > 1e-14 * s0) {
+    for (int k = 0; k < 3; ++k) u1[k] = b[k] / s1;
+  } else {
+    /* collapsed triangle (A-9: several results are correct): any unit vector orthogonal to u0 */
+    double e[3] = {0,0,0};
+    int m = 0; if (fabs(u0[1]) < fabs(u0[m])) m = 1; if (fabs(u0[2]) < fabs(u0[m])) m = 2;
+    e[m] = 1.0;
+    double d = dot3(e, u0);
+    for (int k = 0; k < 3; ++k) u1[k] = e[k] - d*u0[k];
+    double nn = norm3(u1);
+    for (int k = 0; k < 3; ++k) u1[k] /= nn;
+  }
+  for (int k = 0; k < 3; ++k) { U[2*k] = u0[k]; U[2*k+1] = u1[k]; }
+  S[0] = s0; S[1] = s1;
+  V[0] = v00; V[1] = v01; V[2] = v10; V[3] = v11;
+}
+
+/* P = U diag(d) V^T, row-major 3x2 */
+static void compose32(const double *U, const double *d, const double *V, double *P) {
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 2; ++j)
+      P[2*i+j] = U[2*i]*d[0]*V[2*j] + U[2*i+1]*d[1]*V[2*j+1];
+}
+
+/* ---------------------------------------------------------------- local projections
+ * strain: P_s = U diag(clamp(sigma_i,[s_min,s_max])) V^T */
+void oracle_project_strain(const double *F, double s_min, double s_max, double *P) {
+  double U[6], S[2], V[4], d[2];
+  oracle_svd32(F, U, S, V);
+  d[0] = clampd(S[0], s_min, s_max);
+  d[1] = clampd(S[1], s_min, s_max);
+  compose32(U, d, V, P);
+}
+
+/* Closest point (o[0],o[1]) of the hyperbola branch {s1*s2 = a, s > 0} to (sg1,sg2), sg1 >= sg2.
+ * Parametrise s = (q e^t, q e^-t), q = sqrt(a); phi(t) = (q e^t - sg1)^2 + (q e^-t - sg2)^2.
+ * phi(t) <= phi(-t) for t >= 0 when sg1 >= sg2, so the global minimiser has t >= 0; there
+ * phi'(0) = -2q(sg1-sg2) <= 0, phi' > 0 beyond t_hi, and phi' has a single sign change on
+ * t >= 0 (the other normals from an interior point land on t < 0).  The root of phi' is found by
+ * bracketed Newton (bisection whenever Newton leaves the bracket) to 1e-15.  The tests pin the
+ * result against a brute-force scan of the whole branch (both signs of t).
+ * (A-10: a tie sg1 == sg2 > 2q has two mirror minimisers; either is correct.) */
+static double hyp_dphi(double t, double q, double s1, double s2) {
+  double e = exp(t), ei = exp(-t);
+  return e*(q*e - s1) - ei*(q*ei - s2);        /* phi'(t) / (2q) */
+}
+static double hyp_ddphi(double t, double q, double s1, double s2) {
+  double e = exp(t), ei = exp(-t);
+  return 2*q*e*e - s1*e + 2*q*ei*ei - s2*ei;   /* phi''(t) / (2q) */
+}
+void oracle_closest_on_hyperbola(double sg1, double sg2, double a, double *o) {
+  double q = sqrt(a);
+  double lo = 0.0, hi = log((sg1 > q ? sg1 : q) / q) + 1.0;   /* phi'(hi) > 0 */
+  double t;
+  if (hyp_dphi(lo, q, sg1, sg2) >= 0.0) {
+    t = lo;                                     /* sg1 == sg2 <= 2q: minimiser at t = 0 ... */
+    if (sg1 == sg2 && sg1 > 2.0*q) {            /* ... unless t = 0 is the local maximum (A-10) */
+      double e = (sg1 + sqrt(sg1*sg1 - 4.0*q*q)) / (2.0*q);
+      t = log(e);
+    }
+  } else {
+    t = 0.5 * log((sg1 > 0 && sg2 > 0) ? sg1 / sg2 : 1.0);     /* same-ratio point as a start */
+    if (!(t > lo && t < hi)) t = 0.5 * (lo + hi);
+    for (int it = 0; it < 200; ++it) {
+      double f = hyp_dphi(t, q, sg1, sg2);
+      if (f == 0.0) break;
+      if (f < 0.0) lo = t; else hi = t;
+      double df = hyp_ddphi(t, q, sg1, sg2);
+      double tn = (df > 0.0) ? t - f / df : lo - 1.0;
+      if (!(tn > lo && tn < hi)) tn = 0.5 * (lo + hi);
+      double step = fabs(tn - t);
+      t = tn;
+      if (step <= 1e-15 * (1.0 + fabs(t))) break;
+    }
+  }
+  o[0] = q * exp(t); o[1] = q * exp(-t);
+}
+
+/* area: a* = clamp(s1 s2,[a_min,a_max]); P_a = F if s1 s2 == a*, else U diag(s') V^T with s' the
+ * closest point of {s1 s2 = a*} to (sigma1, sigma2) */
+void oracle_project_area(const double *F, double a_min, double a_max, double *P) {
+  double U[6], S[2], V[4], d[2];
+  oracle_svd32(F, U, S, V);
+  double prod = S[0] * S[1];
+  double astar = clampd(prod, a_min, a_max);
+  if (prod == astar) { memcpy(P, F, 6 * sizeof(double)); return; }
+  oracle_closest_on_hyperbola(S[0], S[1], astar, d);
+  compose32(U, d, V, P);
+}
+
+/* bending: P_b = r k/||k||; if ||k|| < 1e-30, P_b = k (no force) */
+void oracle_project_bend(const double *k, double r, double *P) {
+  double nk = norm3(k);
+  if (nk < 1e-30) { P[0] = k[0]; P[1] = k[1]; P[2] = k[2]; return; }
+  for (int i = 0; i < 3; ++i) P[i] = r * k[i] / nk;
+}
+
+/* volume: P_v = configuration closest to x (Euclidean over all 3n coordinates) with V(P_v) = V*,
+ * by D <- ((g.D - C)/(g.g)) g, C = V(x+D) - V*, g = grad V(x+D), from D = 0
+ * until |C| < 1e-14 V0 and D has stopped moving
+ * V and grad V of a CLOSED surface are translation invariant (create checks closedness), so they
+ * are evaluated in coordinates translated by -x[vertex 0]: same numbers in exact arithmetic,
+ * no 1e6-sized cancelling terms for a cell that sits 100 um from the origin.
+ * returns the number of iterations used. */
+double oracle_volume_closed(int n, int T, const int32_t *tris, const double *x) {
+  double *y = (double*)malloc(sizeof(double) * 3 * (size_t)n);
+  for (int v = 0; v < n; ++v) for (int d = 0; d < 3; ++d) y[3*v+d] = x[3*v+d] - x[d];
+  double V = oracle_volume(T, tris, y);
+  free(y);
+  return V;
+}
+
+int oracle_project_volume(int n, int T, const int32_t *tris, const double *x, double Vstar,
+                          double V0, double *P) {
+  size_t m = 3 * (size_t)n;
+  double *D = (double*)calloc(m, sizeof(double));
+  double *g = (double*)malloc(m * sizeof(double));
+  double *y = (double*)malloc(m * sizeof(double));
+  int it = 0;
+  for (int v = 0; v < n; ++v) for (int d = 0; d < 3; ++d) y[3*v+d] = x[3*v+d] - x[d];
+  if (oracle_volume(T, tris, y) != Vstar) {
+    for (it = 1; it <= 100; ++it) {
+      double C = oracle_volume(T, tris, y) - Vstar;
+      oracle_volume_grad(n, T, tris, y, g);
+      double gD = 0, gg = 0;
+      for (size_t i = 0; i < m; ++i) { gD += g[i]*D[i]; gg += g[i]*g[i]; }
+      double lam = (gD - C) / gg;
+      double move = 0, size = 0;
+      for (size_t i = 0; i < m; ++i) {
+        double Dn = lam * g[i];
+        double y0 = y[i] - D[i];                        /* translated x */
+        move += (Dn - D[i]) * (Dn - D[i]); size += y0*y0;
+        D[i] = Dn; y[i] = y0 + Dn;
+      }
+      if (fabs(C) < 1e-14 * fabs(V0) && sqrt(move) <= 1e-15 * sqrt(size)) break;
+    }
+  }
+  for (size_t i = 0; i < m; ++i) P[i] = x[i] + D[i];
+  free(D); free(g); free(y);
+  return it;
+}
+
+/* ---------------------------------------------------------------- create (per cell type) */
+static double cot_at(const double *p, const double *q, const double *r) {
+  double u[3], v[3], c[3]; sub3(q, p, u); sub3(r, p, v); cross3(u, v, c);
+  return dot3(u, v) / norm3(c);
+}
+
+/* dense Cholesky A = L L^T (lower), returns 0 on success */
+static int chol_dense(int n, const double *A, double *L) {
+  memset(L, 0, sizeof(double) * (size_t)n * n);
+  for (int j = 0; j < n; ++j) {
+    double d = A[(size_t)j*n + j];
+    for (int k = 0; k < j; ++k) d -= L[(size_t)j*n + k] * L[(size_t)j*n + k];
+    if (!(d > 0.0)) return -1;
+    d = sqrt(d);
+    L[(size_t)j*n + j] = d;
+    for (int i = j + 1; i < n; ++i) {
+      double s = A[(size_t)i*n + j];
+      for (int k = 0; k < j; ++k) s -= L[(size_t)i*n + k] * L[(size_t)j*n + k];
+      L[(size_t)i*n + j] = s / d;
+    }
+  }
+  return 0;
+}
+
+void oracle_destroy(oracle_cell *c) {
+  if (!c) return;
+  free(c->tris); free(c->X); free(c->G); free(c->area); free(c->mass); free(c->hinge);
+  free(c->K); free(c->w_h); free(c->r_h); free(c->A); free(c->L); free(c->LT); free(c);
+}
+
+int oracle_create(int n, int T, const int32_t *tris, const double *X, const oracle_material *mat,
+                  double h, oracle_cell **out) {
+  if (!out) return ORACLE_EINVAL;
+  *out = NULL;
+  if (n < 4 || T < 4 || !tris || !X || !mat || !(h > 0)) return ORACLE_EINVAL;
+  if (mat->s_min > mat->s_max || mat->a_min > mat->a_max || mat->v_min > mat->v_max) return ORACLE_EINVAL;
+  if (mat->c_alpha != 0.0 || mat->c_beta != 0.0) return ORACLE_EINVAL;          /* A-5 */
+  if (!(mat->cell_mass > 0)) return ORACLE_EINVAL;
+  for (int i = 0; i < 3*T; ++i) if (tris[i] < 0 || tris[i] >= n) return ORACLE_EINVAL;
+  if ((3*T) % 2) return ORACLE_EINVAL;
+  int H = 3*T/2;
+
+  oracle_cell *c = (oracle_cell*)calloc(1, sizeof(oracle_cell));
+  if (!c) return ORACLE_ENOMEM;
+  c->n = n; c->T = T; c->H = H; c->mat = *mat; c->h = h;
+  c->tris = (int32_t*)malloc(sizeof(int32_t)*3*T);
+  c->X = (double*)malloc(sizeof(double)*3*n);
+  c->G = (double*)malloc(sizeof(double)*6*T);
+  c->area = (double*)malloc(sizeof(double)*T);
+  c->mass = (double*)calloc(n, sizeof(double));
+  c->hinge = (int32_t*)malloc(sizeof(int32_t)*4*H);
+  c->K = (double*)malloc(sizeof(double)*4*H);
+  c->w_h = (double*)malloc(sizeof(double)*H);
+  c->r_h = (double*)malloc(sizeof(double)*H);
+  c->A = (double*)calloc((size_t)n*n, sizeof(double));
+  c->L = (double*)malloc(sizeof(double)*(size_t)n*n);
+  c->LT = (double*)malloc(sizeof(double)*(size_t)n*n);
+  memcpy(c->tris, tris, sizeof(int32_t)*3*T);
+  memcpy(c->X, X, sizeof(double)*3*n);
+
+  /* A-14: closed, consistently oriented 2-manifold: every directed edge exactly once and its
+   * reverse exactly once.  opp[u*n+v] = vertex opposite directed edge u->v, or -1. */
+  int32_t *opp = (int32_t*)malloc(sizeof(int32_t)*(size_t)n*n);
+  for (size_t i = 0; i < (size_t)n*n; ++i) opp[i] = -1;
+  int bad = 0;
+  for (int t = 0; t < T && !bad; ++t) {
+    for (int e = 0; e < 3; ++e) {
+      int u = tris[3*t+e], v = tris[3*t+(e+1)%3], w = tris[3*t+(e+2)%3];
+      if (u == v || opp[(size_t)u*n+v] != -1) { bad = 1; break; }
+      opp[(size_t)u*n+v] = w;
+    }
+  }
+  for (int t = 0; t < T && !bad; ++t)
+    for (int e = 0; e < 3; ++e) {
+      int u = tris[3*t+e], v = tris[3*t+(e+1)%3];
+      if (opp[(size_t)v*n+u] == -1) { bad = 1; break; }
+    }
+  if (bad) { free(opp); oracle_destroy(c); return ORACLE_EINVAL; }
+
+  /* step 1: per-triangle rest frame, D_m, rest area, G_t = D_m^-T [[-1,1,0],[-1,0,1]] */
+  double total_area = 0.0;
+  for (int t = 0; t < T; ++t) {
+    const double *Xa = X + 3*tris[3*t], *Xb = X + 3*tris[3*t+1], *Xc = X + 3*tris[3*t+2];
+    double e1[3], e2[3], nrm[3], t1[3], t2[3];
+    sub3(Xb, Xa, e1); sub3(Xc, Xa, e2); cross3(e1, e2, nrm);
+    double nn = norm3(nrm), l1 = norm3(e1);
+    if (!(nn > 0) || !(l1 > 0)) { free(opp); oracle_destroy(c); return ORACLE_EINVAL; }
+    for (int k = 0; k < 3; ++k) { nrm[k] /= nn; t1[k] = e1[k] / l1; }
+    cross3(nrm, t1, t2);
+    double d00 = dot3(e1, t1), d01 = dot3(e2, t1), d11 = dot3(e2, t2);   /* D_m = [[d00,d01],[0,d11]] */
+    c->area[t] = 0.5 * nn;
+    total_area += c->area[t];
+    /* D_m^-1 = [[1/d00, -d01/(d00 d11)],[0, 1/d11]];  D_m^-T = its transpose */
+    double i00 = 1.0/d00, i01 = -d01/(d00*d11), i11 = 1.0/d11;
+    double DmInvT[2][2] = {{i00, 0.0}, {i01, i11}};
+    double S[2][3] = {{-1, 1, 0}, {-1, 0, 1}};
+    for (int a = 0; a < 2; ++a)
+      for (int v = 0; v < 3; ++v)
+        c->G[6*t + 3*a + v] = DmInvT[a][0]*S[0][v] + DmInvT[a][1]*S[1][v];
+  }
+  /* step 2: lumped masses m_v = cell_mass a_v / sum a_v, a_v = 1/3 sum_{t contains v} A_t   (A-4) */
+  for (int t = 0; t < T; ++t)
+    for (int e = 0; e < 3; ++e) c->mass[tris[3*t+e]] += c->area[t] / 3.0;
+  for (int v = 0; v < n; ++v) c->mass[v] = mat->cell_mass * c->mass[v] / total_area;
+
+  /* step 3: hinges, one per undirected edge in increasing (min,max) order */
+  int hcount = 0;
+  for (int u = 0; u < n; ++u)
+    for (int v = u + 1; v < n; ++v) {
+      if (opp[(size_t)u*n+v] == -1) continue;
+      int x2 = opp[(size_t)u*n+v], x3 = opp[(size_t)v*n+u];
+      if (hcount >= H) { free(opp); oracle_destroy(c); return ORACLE_EINVAL; }
+      int32_t *st = c->hinge + 4*hcount;
+      st[0] = u; st[1] = v; st[2] = x2; st[3] = x3;
+      const double *X0 = X+3*u, *X1 = X+3*v, *X2 = X+3*x2, *X3 = X+3*x3;
+      double c01 = cot_at(X0, X1, X2), c02 = cot_at(X0, X1, X3);
+      double c03 = cot_at(X1, X0, X2), c04 = cot_at(X1, X0, X3);
+      double *K = c->K + 4*hcount;
+      K[0] = c03 + c04; K[1] = c01 + c02; K[2] = -c01 - c03; K[3] = -c02 - c04;
+      double a[3], b[3], cr[3];
+      sub3(X1, X0, a); sub3(X2, X0, b); cross3(a, b, cr); double A0 = 0.5*norm3(cr);
+      sub3(X3, X0, b); cross3(a, b, cr); double A1 = 0.5*norm3(cr);
+      c->w_h[hcount] = mat->k_bend * 3.0 / (A0 + A1);
+      double kv[3] = {0,0,0};
+      for (int i = 0; i < 4; ++i) for (int k = 0; k < 3; ++k) kv[k] += K[i] * X[3*st[i]+k];
+      c->r_h[hcount] = norm3(kv);
+      ++hcount;
+    }
+  free(opp);
+  if (hcount != H) { oracle_destroy(c); return ORACLE_EINVAL; }
+
+  /* step 4: rest volume */
+  c->V0 = oracle_volume(T, tris, X);
+  if (!(c->V0 > 0)) { oracle_destroy(c); return ORACLE_EINVAL; }
+
+  /* step 5: A_sys = diag(m)/h^2 + sum_t (w_s+w_a) G^T G + sum_h w_h K^T K + w_volume I */
+  for (int v = 0; v < n; ++v) c->A[(size_t)v*n+v] += c->mass[v] / (h*h) + mat->w_volume;
+  for (int t = 0; t < T; ++t) {
+    double w = (mat->k_strain + mat->k_area) * c->area[t];
+    const double *G = c->G + 6*t;
+    for (int p = 0; p < 3; ++p)
+      for (int q = 0; q < 3; ++q)
+        c->A[(size_t)tris[3*t+p]*n + tris[3*t+q]] += w * (G[p]*G[q] + G[3+p]*G[3+q]);
+  }
+  for (int hh = 0; hh < H; ++hh) {
+    const int32_t *st = c->hinge + 4*hh; const double *K = c->K + 4*hh;
+    for (int p = 0; p < 4; ++p)
+      for (int q = 0; q < 4; ++q)
+        c->A[(size_t)st[p]*n + st[q]] += c->w_h[hh] * K[p] * K[q];
+  }
+  if (chol_dense(n, c->A, c->L) != 0) { oracle_destroy(c); return ORACLE_EINVAL; }
+  for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) c->LT[(size_t)j*n+i] = c->L[(size_t)i*n+j];
+  *out = c;
+  return ORACLE_OK;
+}
+
+/* getters for the tests */
+int oracle_n_hinges(const oracle_cell *c) { return c->H; }
+double oracle_rest_volume(const oracle_cell *c) { return c->V0; }
+void oracle_get_hinges(const oracle_cell *c, int32_t *o) { memcpy(o, c->hinge, sizeof(int32_t)*4*c->H); }
+void oracle_get_K(const oracle_cell *c, double *o) { memcpy(o, c->K, sizeof(double)*4*c->H); }
+void oracle_get_hinge_weights(const oracle_cell *c, double *w, double *r) {
+  memcpy(w, c->w_h, sizeof(double)*c->H); memcpy(r, c->r_h, sizeof(double)*c->H);
+}
+void oracle_get_masses(const oracle_cell *c, double *o) { memcpy(o, c->mass, sizeof(double)*c->n); }
+void oracle_get_areas(const oracle_cell *c, double *o) { memcpy(o, c->area, sizeof(double)*c->T); }
+void oracle_get_G(const oracle_cell *c, double *o) { memcpy(o, c->G, sizeof(double)*6*c->T); }
+void oracle_get_system(const oracle_cell *c, double *o) { memcpy(o, c->A, sizeof(double)*(size_t)c->n*c->n); }
+
+/* ---------------------------------------------------------------- the step, piece by piece */
+/* F_t (row-major 3x2):  F^T = G [x_a; x_b; x_c] */
+void oracle_deformation_gradient(const oracle_cell *c, int t, const double *x, double *F) {
+  const double *G = c->G + 6*t; const int32_t *tr = c->tris + 3*t;
+  for (int i = 0; i < 3; ++i)
+    for (int a = 0; a < 2; ++a) {
+      double s = 0;
+      for (int v = 0; v < 3; ++v) s += G[3*a+v] * x[3*tr[v]+i];
+      F[2*i+a] = s;
+    }
+}
+
+static void hinge_vector(const oracle_cell *c, int hh, const double *x, double *k) {
+  const int32_t *st = c->hinge + 4*hh; const double *K = c->K + 4*hh;
+  k[0] = k[1] = k[2] = 0;
+  for (int i = 0; i < 4; ++i) for (int d = 0; d < 3; ++d) k[d] += K[i] * x[3*st[i]+d];
+}
+
+/* local step: all projections at x.  Ps, Pa [T][6]; Pb [H][3]; Pv [n][3] */
+void oracle_local(const oracle_cell *c, const double *x, double *Ps, double *Pa, double *Pb, double *Pv) {
+  const oracle_material *m = &c->mat;
+  for (int t = 0; t < c->T; ++t) {
+    double F[6];
+    oracle_deformation_gradient(c, t, x, F);
+    oracle_project_strain(F, m->s_min, m->s_max, Ps + 6*t);
+    oracle_project_area(F, m->a_min, m->a_max, Pa + 6*t);
+  }
+  for (int hh = 0; hh < c->H; ++hh) {
+    double k[3];
+    hinge_vector(c, hh, x, k);
+    oracle_project_bend(k, c->r_h[hh], Pb + 3*hh);
+  }
+  double V = oracle_volume_closed(c->n, c->T, c->tris, x);
+  double Vstar = clampd(V, m->v_min * c->V0, m->v_max * c->V0);
+  oracle_project_volume(c->n, c->T, c->tris, x, Vstar, c->V0, Pv);
+}
+
+/* b = diag(m)/h^2 s + sum_t G^T (w_s Ps^T + w_a Pa^T) + sum_h w_h K^T Pb + w_volume Pv */
+void oracle_rhs(const oracle_cell *c, const double *s, const double *Ps, const double *Pa,
+                const double *Pb, const double *Pv, double *b) {
+  const oracle_material *m = &c->mat;
+  double ih2 = 1.0 / (c->h * c->h);
+  for (int v = 0; v < c->n; ++v)
+    for (int d = 0; d < 3; ++d)
+      b[3*v+d] = c->mass[v] * ih2 * s[3*v+d] + m->w_volume * Pv[3*v+d];
+  for (int t = 0; t < c->T; ++t) {
+    double ws = m->k_strain * c->area[t], wa = m->k_area * c->area[t];
+    const double *G = c->G + 6*t; const int32_t *tr = c->tris + 3*t;
+    for (int v = 0; v < 3; ++v)
+      for (int d = 0; d < 3; ++d)
+        for (int a = 0; a < 2; ++a)
+          b[3*tr[v]+d] += G[3*a+v] * (ws * Ps[6*t + 2*d + a] + wa * Pa[6*t + 2*d + a]);
+  }
+  for (int hh = 0; hh < c->H; ++hh) {
+    const int32_t *st = c->hinge + 4*hh; const double *K = c->K + 4*hh;
+    for (int i = 0; i < 4; ++i)
+      for (int d = 0; d < 3; ++d)
+        b[3*st[i]+d] += c->w_h[hh] * K[i] * Pb[3*hh+d];
+  }
+}
+
+/* global step: x = A_sys^-1 b by forward/backward substitution with the dense factor (3 rhs) */
+void oracle_solve(const oracle_cell *c, const double *b, double *x) {
+  int n = c->n; const double *L = c->L, *LT = c->LT;
+  for (int d = 0; d < 3; ++d) {
+    for (int i = 0; i < n; ++i) {                       /* L y = b */
+      double s = b[3*i+d];
+      for (int k = 0; k < i; ++k) s -= L[(size_t)i*n+k] * x[3*k+d];
+      x[3*i+d] = s / L[(size_t)i*n+i];
+    }
+    for (int i = n - 1; i >= 0; --i) {                  /* L^T x = y */
+      double s = x[3*i+d];
+      for (int k = i + 1; k < n; ++k) s -= LT[(size_t)i*n+k] * x[3*k+d];
+      x[3*i+d] = s / L[(size_t)i*n+i];
+    }
+  }
+}
+
+/* E(x;p) = 1/2 ||x-s||^2_M / h^2 + sum 1/2 w_s ||F-Ps||^2 + sum 1/2 w_a ||F-Pa||^2
+ *        + sum 1/2 w_h ||k-Pb||^2 + 1/2 w_volume ||x-Pv||^2       (pin P-3)
+ * parts[5] receives the five terms if not NULL. */
+double oracle_energy(const oracle_cell *c, const double *x, const double *s, const double *Ps,
+                     const double *Pa, const double *Pb, const double *Pv, double *parts) {
+  const oracle_material *m = &c->mat;
+  double e[5] = {0,0,0,0,0};
+  double ih2 = 1.0 / (c->h * c->h);
+  for (int v = 0; v < c->n; ++v)
+    for (int d = 0; d < 3; ++d) {
+      double u = x[3*v+d] - s[3*v+d], q = x[3*v+d] - Pv[3*v+d];
+      e[0] += 0.5 * c->mass[v] * ih2 * u*u;
+      e[4] += 0.5 * m->w_volume * q*q;
+    }
+  for (int t = 0; t < c->T; ++t) {
+    double F[6]; oracle_deformation_gradient(c, t, x, F);
+    double ds = 0, da = 0;
+    for (int k = 0; k < 6; ++k) {
+      ds += (F[k]-Ps[6*t+k])*(F[k]-Ps[6*t+k]);
+      da += (F[k]-Pa[6*t+k])*(F[k]-Pa[6*t+k]);
+    }
+    e[1] += 0.5 * m->k_strain * c->area[t] * ds;
+    e[2] += 0.5 * m->k_area * c->area[t] * da;
+  }
+  for (int hh = 0; hh < c->H; ++hh) {
+    double k[3]; hinge_vector(c, hh, x, k);
+    double db = 0;
+    for (int d = 0; d < 3; ++d) db += (k[d]-Pb[3*hh+d])*(k[d]-Pb[3*hh+d]);
+    e[3] += 0.5 * c->w_h[hh] * db;
+  }
+  if (parts) memcpy(parts, e, sizeof(e));
+  return e[0] + e[1] + e[2] + e[3] + e[4];
+}
+
+/* internal force f_int(x) = sum w A^T (p(x) - A x)   (pins P-2, P-8) */
+void oracle_fint(const oracle_cell *c, const double *x, double *f) {
+  int n = c->n; const oracle_material *m = &c->mat;
+  double *Ps = (double*)malloc(sizeof(double)*6*c->T), *Pa = (double*)malloc(sizeof(double)*6*c->T);
+  double *Pb = (double*)malloc(sizeof(double)*3*c->H), *Pv = (double*)malloc(sizeof(double)*3*n);
+  double *zero = (double*)calloc(3*(size_t)n, sizeof(double));
+  oracle_local(c, x, Ps, Pa, Pb, Pv);
+  oracle_rhs(c, zero, Ps, Pa, Pb, Pv, f);               /* sum w A^T p */
+  /* minus (sum w A^T A) x = (A_sys - M/h^2) x */
+  double ih2 = 1.0 / (c->h * c->h);
+  for (int i = 0; i < n; ++i)
+    for (int d = 0; d < 3; ++d) {
+      double s = 0;
+      for (int j = 0; j < n; ++j) s += c->A[(size_t)i*n+j] * x[3*j+d];
+      s -= c->mass[i] * ih2 * x[3*i+d];
+      f[3*i+d] -= s;
+    }
+  (void)m;
+  free(Ps); free(Pa); free(Pb); free(Pv); free(zero);
+}
+
+/* One time step of ONE cell (SURVEY.md 8(c) "Step"):
+ *   s = x_n + h v_n + h^2 f/m;  x^0 = s;
+ *   repeat n_iters: local projections at x^k, b, x^{k+1} = A_sys^-1 b;
+ *   x_{n+1} = x^{n_iters};  v_{n+1} = (x_{n+1} - x_n)/h.
+ * Optional outputs: iterates [(n_iters+1)][n][3] (x^0 ... x^{n_iters}) and
+ * energies [2*n_iters]: E(x^k;p^k) after each local step, E(x^{k+1};p^k) after each global step. */
+void oracle_step_cell(const oracle_cell *c, double *pos, double *vel, const double *fext,
+                      int n_iters, double *iterates, double *energies) {
+  int n = c->n; size_t m3 = 3*(size_t)n; double h = c->h;
+  double *s = (double*)malloc(sizeof(double)*m3), *x = (double*)malloc(sizeof(double)*m3);
+  double *b = (double*)malloc(sizeof(double)*m3);
+  double *Ps = (double*)malloc(sizeof(double)*6*c->T), *Pa = (double*)malloc(sizeof(double)*6*c->T);
+  double *Pb = (double*)malloc(sizeof(double)*3*c->H), *Pv = (double*)malloc(sizeof(double)*m3);
+  for (int v = 0; v < n; ++v)
+    for (int d = 0; d < 3; ++d)
+      s[3*v+d] = pos[3*v+d] + h * vel[3*v+d] + h*h * fext[3*v+d] / c->mass[v];
+  memcpy(x, s, sizeof(double)*m3);
+  if (iterates) memcpy(iterates, x, sizeof(double)*m3);
+  for (int k = 0; k < n_iters; ++k) {
+    oracle_local(c, x, Ps, Pa, Pb, Pv);
+    if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL);
+    oracle_rhs(c, s, Ps, Pa, Pb, Pv, b);
+    oracle_solve(c, b, x);
+    if (energies) energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL);
+    if (iterates) memcpy(iterates + (size_t)(k+1)*m3, x, sizeof(double)*m3);
+  }
+  for (size_t i = 0; i < m3; ++i) { vel[i] = (x[i] - pos[i]) / h; pos[i] = x[i]; }
+  free(s); free(x); free(b); free(Ps); free(Pa); free(Pb); free(Pv);
+}
+
+/* All cells of one type, [n_cells][n][3] fp64 arrays, OpenMP over cells only. */
+void oracle_step(const oracle_cell *c, int n_cells, double *pos, double *vel, const double *fext,
+                 int n_iters) {
+  size_t stride = 3*(size_t)c->n;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int i = 0; i < n_cells; ++i)
+    oracle_step_cell(c, pos + i*stride, vel + i*stride, fext + i*stride, n_iters, NULL, NULL);
+}
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
