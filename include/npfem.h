@@ -1,0 +1,167 @@
+/*
+ * npfem.h -- C ABI of the B200-native npFEM solid-phase hot path.
+ *
+ * What the library computes: one nodal projective-FEM time step for many deformable blood cells
+ * of ONE type at once (same surface-mesh topology, rest shape, material, time step).  The step is
+ * the one BASELINE.json's north_star names and PAPER.md describes in words only:
+ *   - PAPER.md:56-60 (Introduction, eq. 2)  elastodynamics of each body, Newton's 2nd law;
+ *   - PAPER.md:66, :70                      "mass-lumped linear FE solver" on triangular surface
+ *                                           meshes, implicit time integration;
+ *   - PAPER.md:90-95 (Implementation)       projective dynamics (ShapeOp lineage), time stepping
+ *                                           after Liu et al.: alternate a LOCAL step (project every
+ *                                           elemental constraint) and a GLOBAL step (solve the
+ *                                           prefactored SPD system shared by all cells of a type);
+ *   - PAPER.md:181                          the energy of a body is a sum of per-element energies,
+ *                                           each with a weight and parameters;
+ *   - PAPER.md:103, :159-163                what crosses the boundary every step (forces in,
+ *                                           positions + velocities out) and the precedent of a
+ *                                           dynamic library driven through ctypes.
+ * The energies themselves (triangle strain, triangle area, bending hinge, cell volume), the
+ * weights and every other point the paper leaves open are the readings A-1..A-16 of DESIGN.md.
+ *
+ * Conventions
+ *   - every function returns NPFEM_OK (0) or a negative error code; no exception crosses the ABI;
+ *     npfem_last_error() returns a thread-local, statically stored message for the last failure;
+ *   - "host" / "device" on each pointer says where the memory lives;
+ *   - units: any consistent system (the harness uses um, us, pg => force nN);
+ *   - vertex order is the CALLER's; the library never renumbers what the caller sees (its internal
+ *     fill/locality permutation is private);
+ *   - npfem_step is asynchronous on the given CUDA stream and allocates nothing.
+ */
+#ifndef NPFEM_H_
+#define NPFEM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NPFEM_OK 0
+#define NPFEM_EINVAL (-1) /* bad argument, non-closed / inconsistently oriented mesh, V0 <= 0,    */
+                          /* degenerate rest triangle, band with min > max, damping != 0          */
+#define NPFEM_ENOMEM (-2) /* host allocation failed                                               */
+#define NPFEM_ECUDA (-3)  /* a CUDA call failed (message holds the CUDA error string)             */
+#define NPFEM_ELIMIT (-4) /* mesh larger than one CTA can hold (n_verts > 1024 or shared memory)  */
+
+typedef struct npfem_handle_s* npfem_handle; /* opaque; one per cell TYPE */
+typedef struct npfem_plan_s* npfem_plan;     /* opaque; host-only create-time data (no CUDA)      */
+
+/* Material of one cell type (A-2..A-5, A-12).  All doubles, caller's unit system.      */
+typedef struct {
+  double cell_mass;              /* total mass, lumped to vertices by rest-area share */
+  double k_strain, s_min, s_max; /* triangle strain weight per rest area; singular-value band       */
+  double k_area, a_min, a_max;   /* triangle area weight per rest area; band on sigma1*sigma2       */
+  double k_bend;                 /* hinge weight, multiplies 3/(A0+A1)                              */
+  double w_volume, v_min, v_max; /* per-cell volume weight; band on V/V0                            */
+  double c_alpha, c_beta;        /* damping (PAPER.md:145,183 Calpha/Cbeta); must be 0 (A-5)        */
+} npfem_material;
+
+/* Tuning knobs that do not change what is computed beyond fp32 rounding.  Pass NULL for defaults. */
+typedef struct {
+  double inv_drop_tol;    /* entries of A_sys^-1 are dropped, smallest first, while the dropped     */
+                          /* l1 mass of a row stays <= inv_drop_tol * ||row||_1.  Default 2^-24     */
+                          /* (below fp32 rounding of the kept sum); < 0 = that default;             */
+                          /* 0 = keep everything (dense operator).                                  */
+  int volume_inner_iters; /* iterations of the volume projection per local step (>= 1); default 2  */
+  int cells_per_cta;      /* 1..5 cells share one CTA and every fetched operator block; 0 = auto   */
+  int global_mode;        /* 0 = auto, 1 = fp32 SIMT blocks, 2 = 3xTF32 tensor-core blocks          */
+} npfem_options;
+
+/*
+ * npfem_create: build everything that depends only on the cell TYPE (rest
+ * operators D_m^-1, rest areas, lumped masses, hinge rows K, rest volume, A_sys = M/h^2 +
+ * sum w A^T A, its inverse in fp64, locality ordering, block-sparse fp32 operator) and upload it.
+ *   n_verts, n_tris  mesh size; closed, consistently oriented 2-manifold (A-14); n_verts <= 1024
+ *   tris             host, int32 [n_tris][3], vertex indices in the caller's numbering
+ *   rest_xyz         host, double [n_verts][3]
+ *   mat              host
+ *   dt               time step h > 0
+ *   cell_stride_floats  floats between consecutive cells in pos/vel/fext; >= 3*n_verts; 0 = the
+ *                    default padded stride (3*n_verts rounded up to a multiple of 4)
+ *   max_cells        upper bound on n_cells of any later npfem_step (sizes nothing today; kept so
+ *                    that npfem_step never allocates whatever the implementation)
+ *   opts             host, may be NULL
+ *   out              receives the handle; the handle owns all device memory it allocates
+ * Errors: NPFEM_EINVAL, NPFEM_ENOMEM, NPFEM_ELIMIT, NPFEM_ECUDA (also when no CUDA device exists:
+ * there is no CPU fallback).
+ */
+int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* rest_xyz,
+                 const npfem_material* mat, double dt, int cell_stride_floats, int max_cells,
+                 const npfem_options* opts, npfem_handle* out);
+
+/*
+ * npfem_step: advance n_cells cells of this type by ONE time step of n_iters local/global
+ * iterations, entirely on the device (one kernel launch, no host round trip; north_star (d)).
+ *   pos, vel  device, float, in/out, [n_cells][cell_stride]; inside a cell vertex-major xyz
+ *             ([n_verts][3]); padding floats are neither read nor written
+ *   fext      device, float, in, same layout: external force per vertex (the fluid/IBM forces of
+ *             PAPER.md:103, generated inputs here)
+ *   n_iters   >= 0 (0 = pure inertial prediction)
+ *   cuda_stream  a cudaStream_t (NULL = default stream); the call only enqueues work
+ * Result: x_{n+1} = x_n + inc, v_{n+1} = inc/h with inc = h v_n + h^2 f/m + d, d the projective-
+ * dynamics correction after n_iters iterations.  Errors: NPFEM_EINVAL,
+ * NPFEM_ECUDA (launch failure).
+ */
+int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+               int n_iters, void* cuda_stream);
+
+/*
+ * npfem_step_host: the same step with HOST buffers (pinned or pageable): cells are cut into
+ * chunks that flow host->device, through the step kernel and device->host on three streams so
+ * copies overlap compute.  Blocking: returns when pos/vel hold the new state.  Uses a device
+ * staging ring owned by the handle (allocated on first use, reused afterwards).
+ *   pos, vel  host, float, in/out, [n_cells][cell_stride];  fext host, in
+ * Bytes moved per call: 3 fields in, 2 fields out, n_cells*cell_stride*4 bytes each.
+ */
+int npfem_step_host(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+                    int n_iters);
+
+int npfem_destroy(npfem_handle h);
+
+const char* npfem_last_error(void); /* thread-local, static storage; never NULL                   */
+int npfem_cell_stride(npfem_handle h); /* floats per cell actually used                           */
+
+/* Introspection of a handle (all host-side, cheap): what the create step decided.               */
+typedef struct {
+  int n_verts, n_tris, n_hinges;
+  int cell_stride;     /* floats */
+  int cells_per_cta;   /* k */
+  int threads_per_cta;
+  int smem_bytes;      /* dynamic shared memory per CTA */
+  int n_vblocks;       /* ceil(n_verts/8): operator is stored as 8x8 blocks */
+  int n_op_blocks;     /* kept 8x8 blocks of A_sys^-1 */
+  int op_nnz;          /* entries of A_sys^-1 kept by the drop rule (before blocking) */
+  int global_mode;     /* 1 = SIMT, 2 = 3xTF32 */
+  int volume_inner_iters;
+  double rest_volume, total_mass, inv_drop_tol;
+} npfem_info;
+int npfem_get_info(npfem_handle h, npfem_info* out);
+
+/*
+ * Host-only half of npfem_create (no CUDA call): used by the CPU tests to check the create-time
+ * logic against the oracle, and by npfem_create itself.  npfem_plan_query copies create-time
+ * arrays out; each `what` below states shape and type.  Returns the number of elements written,
+ * or the number required when `dst` is NULL, or a negative error code.
+ */
+int npfem_plan_create(int n_verts, int n_tris, const int32_t* tris, const double* rest_xyz,
+                      const npfem_material* mat, double dt, const npfem_options* opts,
+                      npfem_plan* out);
+int npfem_plan_destroy(npfem_plan p);
+int npfem_plan_info(npfem_plan p, npfem_info* out);
+#define NPFEM_Q_PERM 1        /* int32 [n_verts]: internal index -> caller vertex                 */
+#define NPFEM_Q_MASS 2        /* double [n_verts]: lumped masses, caller order                     */
+#define NPFEM_Q_SYSTEM 3      /* double [n_verts^2]: A_sys, caller order, row-major                */
+#define NPFEM_Q_OPERATOR 4    /* double [n_verts^2]: the block-sparse fp32 operator expanded back  */
+                              /* to a dense matrix in caller order (dropped entries = 0)           */
+#define NPFEM_Q_HINGE_VERTS 5 /* int32 [n_hinges][4]: (x0,x1,x2,x3) in DESIGN.md's enumeration     */
+#define NPFEM_Q_HINGE_K 6     /* double [n_hinges][4]: cotangent rows                              */
+#define NPFEM_Q_HINGE_WR 7    /* double [n_hinges][2]: (w_h, r_h)                                  */
+#define NPFEM_Q_TRI_DMINV 8   /* double [n_tris][3]: (i00, i01, i11) of D_m^-1                     */
+#define NPFEM_Q_TRI_AREA 9    /* double [n_tris]                                                   */
+int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NPFEM_H_ */

@@ -1,0 +1,319 @@
+// npfem_api.cu -- the C ABI of include/npfem.h: argument checks, handle ownership, uploads,
+// launches and the host-buffer pipeline.  No arithmetic of the method lives here (create-time
+// math: npfem_plan.cpp; step math: npfem_kernels.cu).
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "npfem_internal.h"
+#include "npfem_kernels.cuh"
+
+using namespace npfem;
+
+struct npfem_plan_s {
+  Plan plan;
+};
+
+struct npfem_handle_s {
+  Plan plan;
+  int device = 0;
+  int cell_stride = 0;
+  int max_cells = 0;
+  DevParams dev{};            // device pointers + scalars (pos/vel/fext/n_cells/n_iters set per call)
+  void* blob = nullptr;       // one device allocation holding every constant table
+  // host-buffer pipeline (npfem_step_host)
+  static constexpr int kStages = 3;
+  int chunk_cells = 0;
+  float* stage[kStages][3] = {};   // device staging: pos, vel, fext per stage
+  cudaStream_t streams[kStages] = {};
+  bool pipeline_ready = false;
+};
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int set_err(int code, const std::string& msg) {
+  std::snprintf(g_err, sizeof(g_err), "%s", msg.c_str());
+  return code;
+}
+int cuda_err(cudaError_t e, const char* what) {
+  std::snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+  return NPFEM_ECUDA;
+}
+
+void fill_info(const Plan& P, int cell_stride, npfem_info* o) {
+  o->n_verts = P.n; o->n_tris = P.T; o->n_hinges = P.H;
+  o->cell_stride = cell_stride;
+  o->cells_per_cta = P.cells_per_cta;
+  o->threads_per_cta = P.threads;
+  o->smem_bytes = P.smem_bytes;
+  o->n_vblocks = P.nvb;
+  o->n_op_blocks = (int)P.blk_col.size();
+  o->op_nnz = P.op_nnz;
+  o->global_mode = P.global_mode;
+  o->volume_inner_iters = P.opt.volume_inner_iters;
+  o->rest_volume = P.V0;
+  o->total_mass = P.total_mass;
+  o->inv_drop_tol = P.opt.inv_drop_tol;
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+extern "C" {
+
+const char* npfem_last_error(void) { return g_err; }
+
+int npfem_plan_create(int n_verts, int n_tris, const int32_t* tris, const double* rest_xyz,
+                      const npfem_material* mat, double dt, const npfem_options* opts,
+                      npfem_plan* out) {
+  if (!out) return set_err(NPFEM_EINVAL, "out is NULL");
+  *out = nullptr;
+  npfem_plan_s* p = new (std::nothrow) npfem_plan_s;
+  if (!p) return set_err(NPFEM_ENOMEM, "out of host memory");
+  std::string err;
+  int rc;
+  try {
+    rc = build_plan(n_verts, n_tris, tris, rest_xyz, mat, dt, opts, &p->plan, &err);
+  } catch (const std::bad_alloc&) {
+    delete p;
+    return set_err(NPFEM_ENOMEM, "out of host memory");
+  }
+  if (rc != NPFEM_OK) {
+    delete p;
+    return set_err(rc, err);
+  }
+  *out = p;
+  return NPFEM_OK;
+}
+
+int npfem_plan_destroy(npfem_plan p) {
+  delete p;
+  return NPFEM_OK;
+}
+
+int npfem_plan_info(npfem_plan p, npfem_info* out) {
+  if (!p || !out) return set_err(NPFEM_EINVAL, "null argument");
+  fill_info(p->plan, (3 * p->plan.n + 3) / 4 * 4, out);
+  return NPFEM_OK;
+}
+
+int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems) {
+  if (!p) return set_err(NPFEM_EINVAL, "null plan");
+  const Plan& P = p->plan;
+  const int n = P.n;
+  auto copy_out = [&](const void* src, size_t elems, size_t elem_size) -> int {
+    if (!dst) return (int)elems;
+    if ((size_t)dst_elems < elems) return set_err(NPFEM_EINVAL, "destination too small");
+    std::memcpy(dst, src, elems * elem_size);
+    return (int)elems;
+  };
+  switch (what) {
+    case NPFEM_Q_PERM: return copy_out(P.perm.data(), n, sizeof(int32_t));
+    case NPFEM_Q_MASS: return copy_out(P.mass.data(), n, sizeof(double));
+    case NPFEM_Q_SYSTEM: return copy_out(P.A.data(), (size_t)n * n, sizeof(double));
+    case NPFEM_Q_HINGE_VERTS: return copy_out(P.hinge_verts.data(), 4 * (size_t)P.H, sizeof(int32_t));
+    case NPFEM_Q_HINGE_K: return copy_out(P.hinge_K.data(), 4 * (size_t)P.H, sizeof(double));
+    case NPFEM_Q_HINGE_WR: return copy_out(P.hinge_wr.data(), 2 * (size_t)P.H, sizeof(double));
+    case NPFEM_Q_TRI_DMINV: return copy_out(P.tri_dminv.data(), 3 * (size_t)P.T, sizeof(double));
+    case NPFEM_Q_TRI_AREA: return copy_out(P.tri_area.data(), (size_t)P.T, sizeof(double));
+    case NPFEM_Q_OPERATOR: {
+      const size_t elems = (size_t)n * n;
+      if (!dst) return (int)elems;
+      if ((size_t)dst_elems < elems) return set_err(NPFEM_EINVAL, "destination too small");
+      double* D = static_cast<double*>(dst);
+      std::memset(D, 0, elems * sizeof(double));
+      for (int ib = 0; ib < P.nvb; ++ib)
+        for (int b = P.blk_ptr[ib]; b < P.blk_ptr[ib + 1]; ++b) {
+          const int jb = P.blk_col[b];
+          for (int l = 0; l < 32; ++l)
+            for (int r = 0; r < 2; ++r) {
+              const int j = jb * 8 + (l & 3) + 4 * r, i = ib * 8 + (l >> 2);
+              if (i < n && j < n)
+                D[(size_t)P.perm[i] * n + P.perm[j]] = (double)P.blk_val[(size_t)b * 64 + 2 * l + r];
+            }
+        }
+      return (int)elems;
+    }
+    default: return set_err(NPFEM_EINVAL, "unknown query");
+  }
+}
+
+int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* rest_xyz,
+                 const npfem_material* mat, double dt, int cell_stride_floats, int max_cells,
+                 const npfem_options* opts, npfem_handle* out) {
+  if (!out) return set_err(NPFEM_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (max_cells < 0) return set_err(NPFEM_EINVAL, "max_cells is negative");
+  int stride = cell_stride_floats;
+  if (stride == 0) stride = (3 * n_verts + 3) / 4 * 4;
+  if (stride < 3 * n_verts) return set_err(NPFEM_EINVAL, "cell_stride_floats < 3*n_verts");
+
+  npfem_handle_s* H = new (std::nothrow) npfem_handle_s;
+  if (!H) return set_err(NPFEM_ENOMEM, "out of host memory");
+  std::string err;
+  int rc;
+  try {
+    rc = build_plan(n_verts, n_tris, tris, rest_xyz, mat, dt, opts, &H->plan, &err);
+  } catch (const std::bad_alloc&) {
+    delete H;
+    return set_err(NPFEM_ENOMEM, "out of host memory");
+  }
+  if (rc != NPFEM_OK) {
+    delete H;
+    return set_err(rc, err);
+  }
+  Plan& P = H->plan;
+  H->cell_stride = stride;
+  H->max_cells = max_cells;
+
+  cudaError_t e = cudaGetDevice(&H->device);
+  if (e != cudaSuccess) { delete H; return cuda_err(e, "cudaGetDevice (no CUDA device: there is no CPU fallback)"); }
+  e = configure_kernels(P.smem_bytes);
+  if (e != cudaSuccess) { delete H; return cuda_err(e, "cudaFuncSetAttribute(shared memory)"); }
+
+  // ---- one blob for all constant tables, 256-byte aligned sections
+  const int n = P.n, T = P.T;
+  std::vector<uint16_t> perm16(n), tri_ids(6 * (size_t)T);
+  std::vector<float> tri_f((size_t)kTriFloats * T);
+  for (int i = 0; i < n; ++i) perm16[i] = (uint16_t)P.perm[i];
+  for (int t = 0; t < T; ++t) {
+    for (int q = 0; q < 6; ++q) tri_ids[(size_t)q * T + t] = P.tri[t].ids[q];
+    for (int q = 0; q < kTriFloats; ++q) tri_f[(size_t)q * T + t] = P.tri[t].f[q];
+  }
+  struct Sec { const void* src; size_t bytes; size_t off; };
+  Sec secs[] = {
+      {perm16.data(), perm16.size() * 2, 0},          {tri_ids.data(), tri_ids.size() * 2, 0},
+      {tri_f.data(), tri_f.size() * 4, 0},            {P.h2_over_m.data(), P.h2_over_m.size() * 4, 0},
+      {P.m_over_h2.data(), P.m_over_h2.size() * 4, 0}, {P.inc_ptr.data(), P.inc_ptr.size() * 2, 0},
+      {P.inc_out.data(), P.inc_out.size() * 2, 0},    {P.inc_ring.data(), P.inc_ring.size() * 2, 0},
+      {P.blk_ptr.data(), P.blk_ptr.size() * 4, 0},    {P.blk_col.data(), P.blk_col.size() * 2, 0},
+      {P.blk_val.data(), P.blk_val.size() * 4, 0},
+  };
+  size_t total = 0;
+  for (auto& sct : secs) { sct.off = total; total += align_up(sct.bytes, 256); }
+  e = cudaMalloc(&H->blob, total);
+  if (e != cudaSuccess) { delete H; return cuda_err(e, "cudaMalloc(constants)"); }
+  for (auto& sct : secs) {
+    e = cudaMemcpy(static_cast<char*>(H->blob) + sct.off, sct.src, sct.bytes, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(H->blob); delete H; return cuda_err(e, "cudaMemcpy(constants)"); }
+  }
+  char* base = static_cast<char*>(H->blob);
+  DevParams& D = H->dev;
+  D.n = n; D.T = T; D.nvb = P.nvb; D.k = P.cells_per_cta; D.cell_stride = stride;
+  D.vol_iters = P.opt.volume_inner_iters;
+  D.h = (float)P.h; D.w_volume = (float)P.mat.w_volume; D.V0 = (float)P.V0;
+  D.Vmin = (float)(P.mat.v_min * P.V0); D.Vmax = (float)(P.mat.v_max * P.V0);
+  D.s_min = (float)P.mat.s_min; D.s_max = (float)P.mat.s_max;
+  D.a_min = (float)P.mat.a_min; D.a_max = (float)P.mat.a_max;
+  D.perm = reinterpret_cast<const uint16_t*>(base + secs[0].off);
+  D.tri_ids = reinterpret_cast<const uint16_t*>(base + secs[1].off);
+  D.tri_f = reinterpret_cast<const float*>(base + secs[2].off);
+  D.h2_over_m = reinterpret_cast<const float*>(base + secs[3].off);
+  D.m_over_h2 = reinterpret_cast<const float*>(base + secs[4].off);
+  D.inc_ptr = reinterpret_cast<const uint16_t*>(base + secs[5].off);
+  D.inc_out = reinterpret_cast<const uint16_t*>(base + secs[6].off);
+  D.inc_ring = reinterpret_cast<const uint16_t*>(base + secs[7].off);
+  D.blk_ptr = reinterpret_cast<const int*>(base + secs[8].off);
+  D.blk_col = reinterpret_cast<const uint16_t*>(base + secs[9].off);
+  D.blk_val = reinterpret_cast<const float*>(base + secs[10].off);
+  D.L = smem_layout(n, T, P.nvb, P.cells_per_cta);
+  *out = H;
+  return NPFEM_OK;
+}
+
+int npfem_get_info(npfem_handle h, npfem_info* out) {
+  if (!h || !out) return set_err(NPFEM_EINVAL, "null argument");
+  fill_info(h->plan, h->cell_stride, out);
+  return NPFEM_OK;
+}
+
+int npfem_cell_stride(npfem_handle h) {
+  if (!h) return set_err(NPFEM_EINVAL, "null handle");
+  return h->cell_stride;
+}
+
+int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+               int n_iters, void* cuda_stream) {
+  if (!h) return set_err(NPFEM_EINVAL, "null handle");
+  if (n_cells < 0 || n_iters < 0) return set_err(NPFEM_EINVAL, "negative n_cells or n_iters");
+  if (n_cells == 0) return NPFEM_OK;
+  if (!pos || !vel || !fext) return set_err(NPFEM_EINVAL, "null device pointer");
+  DevParams p = h->dev;
+  p.n_cells = n_cells; p.n_iters = n_iters;
+  p.pos = pos; p.vel = vel; p.fext = fext;
+  cudaError_t e = launch_step(p, h->plan.threads, h->plan.smem_bytes, h->plan.global_mode,
+                              static_cast<cudaStream_t>(cuda_stream));
+  if (e != cudaSuccess) return cuda_err(e, "npfem_step launch");
+  return NPFEM_OK;
+}
+
+int npfem_step_host(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+                    int n_iters) {
+  if (!h) return set_err(NPFEM_EINVAL, "null handle");
+  if (n_cells < 0 || n_iters < 0) return set_err(NPFEM_EINVAL, "negative n_cells or n_iters");
+  if (n_cells == 0) return NPFEM_OK;
+  if (!pos || !vel || !fext) return set_err(NPFEM_EINVAL, "null host pointer");
+  const size_t cell_bytes = (size_t)h->cell_stride * sizeof(float);
+  cudaError_t e;
+  if (!h->pipeline_ready) {
+    // chunk = a whole number of CTAs' worth of cells, about 32 MB per field
+    int chunk = (int)((32u << 20) / cell_bytes);
+    chunk = chunk / h->plan.cells_per_cta * h->plan.cells_per_cta;
+    if (chunk < h->plan.cells_per_cta) chunk = h->plan.cells_per_cta;
+    h->chunk_cells = chunk;
+    for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
+      e = cudaStreamCreateWithFlags(&h->streams[sidx], cudaStreamNonBlocking);
+      if (e != cudaSuccess) return cuda_err(e, "cudaStreamCreate");
+      for (int f = 0; f < 3; ++f) {
+        e = cudaMalloc(&h->stage[sidx][f], (size_t)chunk * cell_bytes);
+        if (e != cudaSuccess) return cuda_err(e, "cudaMalloc(staging)");
+      }
+    }
+    h->pipeline_ready = true;
+  }
+  const int chunk = h->chunk_cells;
+  int idx = 0;
+  for (int c0 = 0; c0 < n_cells; c0 += chunk, ++idx) {
+    const int sidx = idx % npfem_handle_s::kStages;
+    const int nc = (n_cells - c0 < chunk) ? (n_cells - c0) : chunk;
+    const size_t off = (size_t)c0 * h->cell_stride, bytes = (size_t)nc * cell_bytes;
+    cudaStream_t st = h->streams[sidx];
+    // stream order serialises reuse of this stage's buffers with its previous chunk
+    e = cudaMemcpyAsync(h->stage[sidx][0], pos + off, bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->stage[sidx][1], vel + off, bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->stage[sidx][2], fext + off, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_err(e, "cudaMemcpyAsync(H2D)");
+    int rc = npfem_step(h, nc, h->stage[sidx][0], h->stage[sidx][1], h->stage[sidx][2], n_iters, st);
+    if (rc != NPFEM_OK) return rc;
+    e = cudaMemcpyAsync(pos + off, h->stage[sidx][0], bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(vel + off, h->stage[sidx][1], bytes, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_err(e, "cudaMemcpyAsync(D2H)");
+  }
+  for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
+    e = cudaStreamSynchronize(h->streams[sidx]);
+    if (e != cudaSuccess) return cuda_err(e, "cudaStreamSynchronize");
+  }
+  return NPFEM_OK;
+}
+
+int npfem_destroy(npfem_handle h) {
+  if (!h) return NPFEM_OK;
+  if (h->pipeline_ready) {
+    for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
+      for (int f = 0; f < 3; ++f)
+        if (h->stage[sidx][f]) cudaFree(h->stage[sidx][f]);
+      if (h->streams[sidx]) cudaStreamDestroy(h->streams[sidx]);
+    }
+  }
+  if (h->blob) cudaFree(h->blob);
+  delete h;
+  return NPFEM_OK;
+}
+
+}  // extern "C"

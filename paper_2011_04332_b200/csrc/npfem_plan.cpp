@@ -1,0 +1,471 @@
+// npfem_plan.cpp -- host-side, fp64 "create" step of the npFEM hot path.
+//
+// Builds, once per cell TYPE, everything the step kernel treats as constant:
+//   rest operators D_m^-1, rest areas and corner cotangents   (per-element energies
+//   lumped masses                                              with a weight and parameters; :66
+//   hinge rows K, weights w_h, rest magnitudes r_h             mass lumping; readings A-2..A-4)
+//   A_sys = M/h^2 + sum w A^T A + w_volume I                   (north_star: the shared SPD system)
+//   T = A_sys^-1 in fp64, a locality ordering of the vertices, and T cut into 8x8 blocks with the
+//   numerically negligible ones dropped.
+// No CUDA here: this file is plain C++ so that the CPU tests can exercise it through
+// npfem_plan_create / npfem_plan_query.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <deque>
+#include <numeric>
+
+#include "npfem_internal.h"
+
+namespace npfem {
+namespace {
+
+struct V3 {
+  double x, y, z;
+};
+inline V3 operator-(V3 a, V3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
+inline V3 operator+(V3 a, V3 b) { return {a.x + b.x, a.y + b.y, a.z + b.z}; }
+inline V3 operator*(double s, V3 a) { return {s * a.x, s * a.y, s * a.z}; }
+inline double dot(V3 a, V3 b) { return a.x * b.x + a.y * b.y + a.z * b.z; }
+inline V3 cross(V3 a, V3 b) {
+  return {a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+inline double norm(V3 a) { return std::sqrt(dot(a, a)); }
+
+// cotangent of the angle at p between (q - p) and (r - p)
+inline double cot_corner(V3 p, V3 q, V3 r) {
+  V3 u = q - p, v = r - p;
+  return dot(u, v) / norm(cross(u, v));
+}
+
+// ---------------------------------------------------------------- vertex ordering
+// Recursive graph bisection: inside a vertex subset, breadth-first distances from a
+// pseudo-peripheral vertex split the subset into a near and a far half (the cut is moved to a
+// multiple of 8 when the subset is large enough), recursively.  Consecutive groups of 8/16/32
+// internal indices are then compact surface patches, which is what keeps the 8x8 blocks of the
+// numerically sparse A_sys^-1 few.
+struct Bisector {
+  const std::vector<std::vector<int>>& adj;
+  std::vector<int> mark, dist;
+  int stamp = 0;
+  explicit Bisector(const std::vector<std::vector<int>>& a)
+      : adj(a), mark(a.size(), 0), dist(a.size(), 0) {}
+
+  // BFS restricted to vertices with mark == tag; returns visit order
+  std::vector<int> bfs(int src, int tag, const std::vector<int>& tagv) {
+    std::vector<int> order;
+    ++stamp;
+    std::deque<int> q;
+    q.push_back(src);
+    dist[src] = stamp;
+    order.push_back(src);
+    while (!q.empty()) {
+      int u = q.front();
+      q.pop_front();
+      for (int v : adj[u]) {
+        if (tagv[v] == tag && dist[v] != stamp) {
+          dist[v] = stamp;
+          q.push_back(v);
+          order.push_back(v);
+        }
+      }
+    }
+    return order;
+  }
+
+  void run(std::vector<int> verts, std::vector<int>& tagv, int& next_tag, std::vector<int>& out) {
+    if (verts.size() <= 1) {
+      for (int v : verts) out.push_back(v);
+      return;
+    }
+    int tag = next_tag++;
+    for (int v : verts) tagv[v] = tag;
+    int a = verts[0];
+    std::vector<int> order;
+    for (int sweep = 0; sweep < 4; ++sweep) {
+      order = bfs(a, tag, tagv);
+      a = order.back();
+    }
+    if (order.size() < verts.size()) {   // disconnected remainder: append in given order
+      ++stamp;
+      for (int v : order) dist[v] = stamp;
+      for (int v : verts)
+        if (dist[v] != stamp) order.push_back(v);
+    }
+    size_t half = order.size() / 2;
+    if (order.size() >= 16) {
+      size_t h8 = (half + 7) / 8 * 8;
+      if (h8 < order.size()) half = h8;
+    }
+    std::vector<int> left(order.begin(), order.begin() + half), right(order.begin() + half, order.end());
+    run(std::move(left), tagv, next_tag, out);
+    run(std::move(right), tagv, next_tag, out);
+  }
+};
+
+}  // namespace
+
+int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_material* mat,
+               double dt, const npfem_options* opts, Plan* P, std::string* err) {
+  auto fail = [&](int code, const char* msg) {
+    if (err) *err = msg;
+    return code;
+  };
+  if (!tris || !X || !mat || !P) return fail(NPFEM_EINVAL, "null argument");
+  if (n < 4 || T < 4) return fail(NPFEM_EINVAL, "mesh needs at least 4 vertices and 4 triangles");
+  if (!(dt > 0.0)) return fail(NPFEM_EINVAL, "dt must be positive");
+  if (n > kMaxVerts) return fail(NPFEM_ELIMIT, "n_verts exceeds 1024 (one CTA owns whole cells)");
+  if (mat->s_min > mat->s_max || mat->a_min > mat->a_max || mat->v_min > mat->v_max)
+    return fail(NPFEM_EINVAL, "clamp band with min > max");
+  if (mat->c_alpha != 0.0 || mat->c_beta != 0.0)
+    return fail(NPFEM_EINVAL, "damping (c_alpha, c_beta) must be 0 on the hot path (DESIGN.md A-5)");
+  if (!(mat->cell_mass > 0.0)) return fail(NPFEM_EINVAL, "cell_mass must be positive");
+  if (mat->k_strain < 0 || mat->k_area < 0 || mat->k_bend < 0 || mat->w_volume < 0)
+    return fail(NPFEM_EINVAL, "negative weight");
+  if ((3 * T) % 2) return fail(NPFEM_EINVAL, "odd number of triangle edges: mesh is not closed");
+  for (int i = 0; i < 3 * T; ++i)
+    if (tris[i] < 0 || tris[i] >= n) return fail(NPFEM_EINVAL, "triangle index out of range");
+
+  P->n = n; P->T = T; P->H = 3 * T / 2; P->h = dt; P->mat = *mat;
+  npfem_options o{};
+  o.inv_drop_tol = std::ldexp(1.0, -24);
+  if (opts) {
+    if (opts->inv_drop_tol >= 0.0) o.inv_drop_tol = opts->inv_drop_tol;   // < 0 (or NaN) = default
+    o.volume_inner_iters = opts->volume_inner_iters;
+    o.cells_per_cta = opts->cells_per_cta;
+    o.global_mode = opts->global_mode;
+  }
+  if (o.volume_inner_iters <= 0) o.volume_inner_iters = 2;
+  if (o.volume_inner_iters > 8) o.volume_inner_iters = 8;
+  if (o.cells_per_cta < 0 || o.cells_per_cta > kMaxCellsPerCta)
+    return fail(NPFEM_EINVAL, "cells_per_cta must be 0..5");
+  if (o.global_mode < 0 || o.global_mode > 2) return fail(NPFEM_EINVAL, "global_mode must be 0..2");
+  P->tris_ext.assign(tris, tris + 3 * T);
+  auto Xv = [&](int v) { return V3{X[3 * v], X[3 * v + 1], X[3 * v + 2]}; };
+
+  // ---- A-14: closed, consistently oriented 2-manifold: every directed edge once, its reverse once
+  std::vector<int32_t> etri((size_t)n * n, -1);   // triangle holding directed edge u->v
+  std::vector<int8_t> eslot((size_t)n * n, 0);    // slot of u in that triangle
+  for (int t = 0; t < T; ++t)
+    for (int e = 0; e < 3; ++e) {
+      int u = tris[3 * t + e], v = tris[3 * t + (e + 1) % 3];
+      if (u == v) return fail(NPFEM_EINVAL, "degenerate triangle (repeated vertex)");
+      if (etri[(size_t)u * n + v] != -1)
+        return fail(NPFEM_EINVAL, "directed edge used twice: inconsistent orientation or non-manifold");
+      etri[(size_t)u * n + v] = t;
+      eslot[(size_t)u * n + v] = (int8_t)e;
+    }
+  for (int t = 0; t < T; ++t)
+    for (int e = 0; e < 3; ++e) {
+      int u = tris[3 * t + e], v = tris[3 * t + (e + 1) % 3];
+      if (etri[(size_t)v * n + u] == -1) return fail(NPFEM_EINVAL, "open edge: mesh is not closed");
+    }
+  auto opposite = [&](int u, int v) {   // vertex opposite the directed edge u->v
+    int t = etri[(size_t)u * n + v];
+    int s = eslot[(size_t)u * n + v];
+    return (int)tris[3 * t + (s + 2) % 3];
+  };
+
+  // ---- per-triangle rest data
+  P->tri_dminv.resize(3 * (size_t)T);
+  P->tri_area.resize(T);
+  std::vector<double> cotc(3 * (size_t)T);   // rest cotangent at corner slot s of triangle t
+  double total_area = 0.0;
+  for (int t = 0; t < T; ++t) {
+    V3 a = Xv(tris[3 * t]), b = Xv(tris[3 * t + 1]), c = Xv(tris[3 * t + 2]);
+    V3 e1 = b - a, e2 = c - a, nn = cross(e1, e2);
+    double twoA = norm(nn), l1 = norm(e1);
+    if (!(twoA > 0.0) || !(l1 > 0.0)) return fail(NPFEM_EINVAL, "degenerate rest triangle");
+    // local frame t1 = e1/|e1|, t2 = n x t1:  D_m = [[|e1|, e2.t1], [0, e2.t2]]
+    double d00 = l1, d01 = dot(e2, e1) / l1, d11 = twoA / l1;
+    P->tri_dminv[3 * t + 0] = 1.0 / d00;
+    P->tri_dminv[3 * t + 1] = -d01 / (d00 * d11);
+    P->tri_dminv[3 * t + 2] = 1.0 / d11;
+    P->tri_area[t] = 0.5 * twoA;
+    total_area += 0.5 * twoA;
+    cotc[3 * t + 0] = cot_corner(a, b, c);
+    cotc[3 * t + 1] = cot_corner(b, c, a);
+    cotc[3 * t + 2] = cot_corner(c, a, b);
+  }
+
+  // ---- lumped masses (A-4) and rest volume
+  P->mass.assign(n, 0.0);
+  for (int t = 0; t < T; ++t)
+    for (int e = 0; e < 3; ++e) P->mass[tris[3 * t + e]] += P->tri_area[t] / 3.0;
+  for (int v = 0; v < n; ++v) {
+    if (!(P->mass[v] > 0.0)) return fail(NPFEM_EINVAL, "vertex without triangles");
+    P->mass[v] *= mat->cell_mass / total_area;
+  }
+  P->total_mass = mat->cell_mass;
+  double V0 = 0.0;
+  for (int t = 0; t < T; ++t)
+    V0 += dot(Xv(tris[3 * t]), cross(Xv(tris[3 * t + 1]), Xv(tris[3 * t + 2])));
+  V0 /= 6.0;
+  if (!(V0 > 0.0)) return fail(NPFEM_EINVAL, "rest volume is not positive (inward orientation?)");
+  P->V0 = V0;
+
+  // ---- hinges, one per undirected edge, increasing (min, max)
+  const int H = P->H;
+  P->hinge_verts.resize(4 * (size_t)H);
+  P->hinge_K.resize(4 * (size_t)H);
+  P->hinge_wr.resize(2 * (size_t)H);
+  std::vector<int32_t> hinge_of((size_t)n * n, -1);   // undirected lookup (both orders)
+  int hc = 0;
+  for (int u = 0; u < n; ++u)
+    for (int v = u + 1; v < n; ++v) {
+      if (etri[(size_t)u * n + v] == -1) continue;
+      if (hc >= H) return fail(NPFEM_EINVAL, "edge count does not match 3T/2");
+      int x2 = opposite(u, v), x3 = opposite(v, u);
+      V3 p0 = Xv(u), p1 = Xv(v), p2 = Xv(x2), p3 = Xv(x3);
+      double c01 = cot_corner(p0, p1, p2), c02 = cot_corner(p0, p1, p3);
+      double c03 = cot_corner(p1, p0, p2), c04 = cot_corner(p1, p0, p3);
+      double K[4] = {c03 + c04, c01 + c02, -c01 - c03, -c02 - c04};
+      double A0 = 0.5 * norm(cross(p1 - p0, p2 - p0)), A1 = 0.5 * norm(cross(p1 - p0, p3 - p0));
+      double wh = mat->k_bend * 3.0 / (A0 + A1);
+      V3 kv = K[0] * p0 + K[1] * p1 + K[2] * p2 + K[3] * p3;
+      int32_t* hv = &P->hinge_verts[4 * (size_t)hc];
+      hv[0] = u; hv[1] = v; hv[2] = x2; hv[3] = x3;
+      for (int i = 0; i < 4; ++i) P->hinge_K[4 * (size_t)hc + i] = K[i];
+      P->hinge_wr[2 * (size_t)hc] = wh;
+      P->hinge_wr[2 * (size_t)hc + 1] = norm(kv);
+      hinge_of[(size_t)u * n + v] = hinge_of[(size_t)v * n + u] = hc;
+      ++hc;
+    }
+  if (hc != H) return fail(NPFEM_EINVAL, "edge count does not match 3T/2");
+
+  // ---- A_sys (caller order)
+  const double ih2 = 1.0 / (dt * dt);
+  P->A.assign((size_t)n * n, 0.0);
+  std::vector<double>& A = P->A;
+  for (int v = 0; v < n; ++v) A[(size_t)v * n + v] = P->mass[v] * ih2 + mat->w_volume;
+  for (int t = 0; t < T; ++t) {
+    double i00 = P->tri_dminv[3 * t], i01 = P->tri_dminv[3 * t + 1], i11 = P->tri_dminv[3 * t + 2];
+    // columns of G = D_m^-T [[-1,1,0],[-1,0,1]]: vertex b -> (i00, i01), c -> (0, i11), a -> -(b + c)
+    double G[3][2] = {{-i00, -i01 - i11}, {i00, i01}, {0.0, i11}};
+    double w = (mat->k_strain + mat->k_area) * P->tri_area[t];
+    for (int p = 0; p < 3; ++p)
+      for (int q = 0; q < 3; ++q)
+        A[(size_t)tris[3 * t + p] * n + tris[3 * t + q]] += w * (G[p][0] * G[q][0] + G[p][1] * G[q][1]);
+  }
+  for (int hh = 0; hh < H; ++hh) {
+    const int32_t* hv = &P->hinge_verts[4 * (size_t)hh];
+    const double* K = &P->hinge_K[4 * (size_t)hh];
+    double wh = P->hinge_wr[2 * (size_t)hh];
+    for (int p = 0; p < 4; ++p)
+      for (int q = 0; q < 4; ++q) A[(size_t)hv[p] * n + hv[q]] += wh * K[p] * K[q];
+  }
+
+  // ---- T = A_sys^-1 (fp64): Cholesky A = L L^T, M = L^-1, T = M^T M
+  std::vector<double> L((size_t)n * n, 0.0), M((size_t)n * n, 0.0), Tinv((size_t)n * n, 0.0);
+  for (int j = 0; j < n; ++j) {
+    for (int i = j; i < n; ++i) {
+      double s = A[(size_t)i * n + j];
+      const double *li = &L[(size_t)i * n], *lj = &L[(size_t)j * n];
+      for (int k = 0; k < j; ++k) s -= li[k] * lj[k];
+      if (i == j) {
+        if (!(s > 0.0)) return fail(NPFEM_EINVAL, "system matrix is not positive definite");
+        L[(size_t)j * n + j] = std::sqrt(s);
+      } else {
+        L[(size_t)i * n + j] = s / L[(size_t)j * n + j];
+      }
+    }
+  }
+  for (int i = 0; i < n; ++i) {
+    double* mi = &M[(size_t)i * n];
+    mi[i] = 1.0;
+    for (int k = 0; k < i; ++k) {
+      double lik = L[(size_t)i * n + k];
+      if (lik == 0.0) continue;
+      const double* mk = &M[(size_t)k * n];
+      for (int j = 0; j <= k; ++j) mi[j] -= lik * mk[j];
+    }
+    double inv = 1.0 / L[(size_t)i * n + i];
+    for (int j = 0; j <= i; ++j) mi[j] *= inv;
+  }
+  for (int k = 0; k < n; ++k) {
+    const double* mk = &M[(size_t)k * n];
+    for (int i = 0; i <= k; ++i) {
+      double mki = mk[i];
+      if (mki == 0.0) continue;
+      double* ti = &Tinv[(size_t)i * n];
+      for (int j = 0; j <= i; ++j) ti[j] += mki * mk[j];
+    }
+  }
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < i; ++j) Tinv[(size_t)j * n + i] = Tinv[(size_t)i * n + j];
+  L.clear(); L.shrink_to_fit(); M.clear(); M.shrink_to_fit();
+
+  // ---- locality ordering
+  std::vector<std::vector<int>> adj(n);
+  for (int u = 0; u < n; ++u)
+    for (int v = 0; v < n; ++v)
+      if (etri[(size_t)u * n + v] != -1) adj[u].push_back(v);
+  {
+    Bisector bis(adj);
+    std::vector<int> all(n), tagv(n, 0), order;
+    std::iota(all.begin(), all.end(), 0);
+    int next_tag = 1;
+    order.reserve(n);
+    bis.run(all, tagv, next_tag, order);
+    P->perm.assign(order.begin(), order.end());
+    P->iperm.assign(n, -1);
+    for (int i = 0; i < n; ++i) P->iperm[P->perm[i]] = i;
+    for (int v = 0; v < n; ++v)
+      if (P->iperm[v] < 0) return fail(NPFEM_EINVAL, "internal: ordering is not a permutation");
+  }
+
+  // ---- drop rule on T (per row: smallest entries first while dropped l1 mass <= tol * ||row||_1),
+  //      symmetrised, then 8x8 blocks in internal numbering; kept blocks store ALL their entries
+  const int nvb = (n + 7) / 8;
+  P->nvb = nvb;
+  std::vector<uint8_t> keep((size_t)n * n, 0);
+  {
+    std::vector<int> idx(n);
+    for (int i = 0; i < n; ++i) {
+      const double* ti = &Tinv[(size_t)i * n];
+      double l1 = 0.0;
+      for (int j = 0; j < n; ++j) l1 += std::fabs(ti[j]);
+      std::iota(idx.begin(), idx.end(), 0);
+      std::sort(idx.begin(), idx.end(), [&](int p, int q) {
+        double ap = std::fabs(ti[p]), aq = std::fabs(ti[q]);
+        return ap != aq ? ap < aq : p < q;
+      });
+      double dropped = 0.0;
+      int m = 0;
+      while (m < n && dropped + std::fabs(ti[idx[m]]) <= o.inv_drop_tol * l1 && idx[m] != i) {
+        dropped += std::fabs(ti[idx[m]]);
+        ++m;
+      }
+      for (int q = m; q < n; ++q) keep[(size_t)i * n + idx[q]] = 1;
+      keep[(size_t)i * n + i] = 1;
+    }
+  }
+  int nnz = 0;
+  std::vector<uint8_t> bmask((size_t)nvb * nvb, 0);
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j)
+      if (keep[(size_t)i * n + j] || keep[(size_t)j * n + i]) {
+        ++nnz;
+        bmask[(size_t)(P->iperm[i] / 8) * nvb + P->iperm[j] / 8] = 1;
+      }
+  P->op_nnz = nnz;
+  P->blk_ptr.assign(nvb + 1, 0);
+  P->blk_col.clear();
+  P->blk_val.clear();
+  for (int ib = 0; ib < nvb; ++ib) {
+    for (int jb = 0; jb < nvb; ++jb) {
+      if (!bmask[(size_t)ib * nvb + jb]) continue;
+      P->blk_col.push_back((uint16_t)jb);
+      size_t base = P->blk_val.size();
+      P->blk_val.resize(base + 64, 0.0f);
+      for (int l = 0; l < 32; ++l)
+        for (int r = 0; r < 2; ++r) {
+          int j = jb * 8 + (l & 3) + 4 * r;   // source vertex (k index of the mma B fragment)
+          int i = ib * 8 + (l >> 2);          // output vertex (n index)
+          if (i < n && j < n)
+            P->blk_val[base + 2 * l + r] = (float)Tinv[(size_t)P->perm[i] * n + P->perm[j]];
+        }
+    }
+    P->blk_ptr[ib + 1] = (int32_t)P->blk_col.size();
+  }
+
+  // ---- per-vertex constants and cyclic incidence lists (internal numbering)
+  P->h2_over_m.resize(n);
+  P->m_over_h2.resize(n);
+  for (int i = 0; i < n; ++i) {
+    double m = P->mass[P->perm[i]];
+    P->h2_over_m[i] = (float)(dt * dt / m);
+    P->m_over_h2[i] = (float)(m * ih2);
+  }
+  // internal triangle order: by smallest internal vertex id, then by the sum
+  std::vector<int> torder(T);
+  std::iota(torder.begin(), torder.end(), 0);
+  auto tkey = [&](int t) {
+    int a = P->iperm[tris[3 * t]], b = P->iperm[tris[3 * t + 1]], c = P->iperm[tris[3 * t + 2]];
+    return std::make_pair(std::min(a, std::min(b, c)), a + b + c);
+  };
+  std::sort(torder.begin(), torder.end(), [&](int p, int q) {
+    auto kp = tkey(p), kq = tkey(q);
+    return kp != kq ? kp < kq : p < q;
+  });
+  std::vector<int> tint(T);   // caller triangle -> internal triangle
+  for (int ti = 0; ti < T; ++ti) tint[torder[ti]] = ti;
+
+  P->tri.assign(T, TriConst{});
+  for (int ti = 0; ti < T; ++ti) {
+    int t = torder[ti];
+    TriConst& tc = P->tri[ti];
+    int ve[3] = {tris[3 * t], tris[3 * t + 1], tris[3 * t + 2]};
+    for (int s = 0; s < 3; ++s) tc.ids[s] = (uint16_t)P->iperm[ve[s]];
+    tc.f[0] = (float)P->tri_dminv[3 * t];
+    tc.f[1] = (float)P->tri_dminv[3 * t + 1];
+    tc.f[2] = (float)P->tri_dminv[3 * t + 2];
+    tc.f[3] = (float)(mat->k_strain * P->tri_area[t]);
+    tc.f[4] = (float)(mat->k_area * P->tri_area[t]);
+    for (int e = 0; e < 3; ++e) {
+      int p = ve[e], q = ve[(e + 1) % 3], oo = ve[(e + 2) % 3];
+      int far = opposite(q, p);
+      tc.ids[3 + e] = (uint16_t)P->iperm[far];
+      int hh = hinge_of[(size_t)p * n + q];
+      const int32_t* hv = &P->hinge_verts[4 * (size_t)hh];
+      const double* K = &P->hinge_K[4 * (size_t)hh];
+      double sw = std::sqrt(P->hinge_wr[2 * (size_t)hh]);
+      auto Kof = [&](int vtx) {
+        for (int i = 0; i < 4; ++i)
+          if (hv[i] == vtx) return K[i];
+        return 0.0;
+      };
+      tc.f[5 + 4 * e + 0] = (float)(sw * Kof(p));
+      tc.f[5 + 4 * e + 1] = (float)(sw * Kof(q));
+      tc.f[5 + 4 * e + 2] = (float)(sw * Kof(oo));
+      tc.f[5 + 4 * e + 3] = (float)(sw * P->hinge_wr[2 * (size_t)hh + 1]);
+    }
+  }
+  P->inc_ptr.assign(n + 1, 0);
+  P->inc_out.clear();
+  P->inc_ring.clear();
+  for (int i = 0; i < n; ++i) {
+    int ve = P->perm[i];
+    int t0 = -1, s0 = 0;
+    for (int w : adj[ve]) {
+      t0 = etri[(size_t)ve * n + w];
+      s0 = eslot[(size_t)ve * n + w];
+      break;
+    }
+    int t = t0, s = s0, count = 0;
+    do {
+      int r0 = tris[3 * t + (s + 1) % 3], r1 = tris[3 * t + (s + 2) % 3];
+      P->inc_out.push_back((uint16_t)(tint[t] * 9 + s * 3));
+      P->inc_ring.push_back((uint16_t)P->iperm[r0]);
+      // next triangle around ve holds the directed edge ve -> r1
+      int tn = etri[(size_t)ve * n + r1];
+      s = eslot[(size_t)ve * n + r1];
+      t = tn;
+      if (++count > T) return fail(NPFEM_EINVAL, "non-manifold vertex fan");
+    } while (t != t0);
+    if (count != (int)adj[ve].size()) return fail(NPFEM_EINVAL, "non-manifold vertex (several fans)");
+    P->inc_ptr[i + 1] = (uint16_t)P->inc_out.size();
+  }
+
+  // ---- launch configuration
+  int need = std::max(n, (T + kTrisPerThread - 1) / kTrisPerThread);
+  P->threads = (need + 31) / 32 * 32;
+  if (P->threads > 1024) return fail(NPFEM_ELIMIT, "mesh needs more than 1024 threads per cell");
+  const int smem_max = kSmemMaxDynamic;
+  int k = o.cells_per_cta ? o.cells_per_cta : kMaxCellsPerCta;
+  while (k > 1 && smem_layout(n, T, nvb, k).total > smem_max) {
+    if (o.cells_per_cta) return fail(NPFEM_ELIMIT, "requested cells_per_cta does not fit shared memory");
+    --k;
+  }
+  if (smem_layout(n, T, nvb, k).total > smem_max)
+    return fail(NPFEM_ELIMIT, "cell state does not fit the shared memory of one SM");
+  P->cells_per_cta = k;
+  P->smem_bytes = smem_layout(n, T, nvb, k).total;
+  P->global_mode = o.global_mode ? o.global_mode : 1;
+  o.cells_per_cta = k;
+  o.global_mode = P->global_mode;
+  P->opt = o;
+  return NPFEM_OK;
+}
+
+}  // namespace npfem

@@ -1,0 +1,53 @@
+"""Device-buffer plumbing around the C ABI: pad [N,V,3] arrays to the cell stride, run steps.
+
+PyTorch is used for device memory and streams only; every step of the method runs in
+libnpfem_b200.so.  No arithmetic of the method lives here.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from .binding import NpfemHandle
+
+
+def to_strided(a: np.ndarray | torch.Tensor, stride: int, device="cuda") -> torch.Tensor:
+    """[N,V,3] float32 -> device tensor [N,stride] (cell-major, vertex-major xyz, zero padding)."""
+    t = torch.as_tensor(a, dtype=torch.float32)
+    n = t.shape[0]
+    flat = t.reshape(n, -1)
+    out = torch.zeros((n, stride), dtype=torch.float32, device=device)
+    out[:, : flat.shape[1]] = flat.to(device)
+    return out
+
+
+def from_strided(t: torch.Tensor, n_verts: int) -> np.ndarray:
+    """device/host tensor [N,stride] -> numpy float32 [N,V,3]."""
+    return t[:, : 3 * n_verts].reshape(t.shape[0], n_verts, 3).cpu().numpy()
+
+
+class DeviceGroup:
+    """One cell type resident on the GPU: handle + pos/vel/fext device buffers."""
+
+    def __init__(self, tris, rest, material, dt, pos0, vel0, device="cuda", **options):
+        self.handle = NpfemHandle(tris, rest, material, dt, 0, int(pos0.shape[0]), **options)
+        self.n_verts = int(rest.shape[0])
+        self.n_cells = int(pos0.shape[0])
+        self.stride = self.handle.cell_stride
+        self.device = device
+        self.pos = to_strided(pos0, self.stride, device)
+        self.vel = to_strided(vel0, self.stride, device)
+        self.fext = torch.zeros_like(self.pos)
+
+    def set_forces(self, f):
+        if isinstance(f, torch.Tensor) and f.is_cuda and f.shape == self.fext.shape:
+            self.fext = f
+        else:
+            self.fext = to_strided(f, self.stride, self.device)
+
+    def step(self, n_iters: int, stream=None):
+        self.handle.step(self.n_cells, self.pos, self.vel, self.fext, n_iters, stream)
+
+    def state(self):
+        torch.cuda.synchronize()
+        return (from_strided(self.pos, self.n_verts), from_strided(self.vel, self.n_verts))
