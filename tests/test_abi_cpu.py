@@ -1,0 +1,157 @@
+"""CPU-only checks of the product's host side (no compute call needs a GPU):
+ - the C-ABI library loads and exports every symbol include/npfem.h declares;
+ - the create-time plan (npfem_plan_*, plain C++ fp64) agrees with the oracle's create step;
+ - the block-sparse operator is A_sys^-1 up to the documented drop rule, and the increment-form
+   algebra the kernel uses reproduces the oracle's iterates when evaluated in fp64;
+ - argument errors come back as error codes, and creating a handle without CUDA fails loudly.
+"""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from oracle import npfem_oracle as O
+from paper_2011_04332_b200 import NpfemError, NpfemHandle, NpfemPlan, load_library
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+DT = 0.1
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "npfem.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(npfem_[a-z_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    names = _declared_functions()
+    assert {"npfem_create", "npfem_step", "npfem_destroy", "npfem_last_error",
+            "npfem_cell_stride", "npfem_step_host"} <= set(names)
+    lib = load_library()
+    for name in names:
+        assert hasattr(lib, name), f"{name} declared in include/npfem.h but not exported"
+        assert ctypes.cast(getattr(lib, name), ctypes.c_void_p).value
+
+
+@pytest.fixture(scope="module", params=[("rbc", 2), ("plt", 1), ("rbc", 3)])
+def cell(request):
+    kind, level = request.param
+    rest, tris = W.rest_shape(kind, level)
+    mat = W.default_material(rest, tris)
+    return rest, tris, mat, NpfemPlan(tris, rest, mat, DT), O.OracleCell(tris, rest, mat, DT)
+
+
+def test_plan_create_step_matches_the_oracle(cell):
+    rest, tris, mat, plan, oc = cell
+    n, T = rest.shape[0], tris.shape[0]
+    info = plan.info()
+    assert (info["n_verts"], info["n_tris"], info["n_hinges"]) == (n, T, 3 * T // 2)
+    assert info["rest_volume"] == pytest.approx(oc.rest_volume, rel=1e-13)
+    assert np.allclose(plan.query("mass"), oc.masses(), rtol=1e-13)
+    assert plan.query("mass").sum() == pytest.approx(mat["cell_mass"], rel=1e-13)
+    assert np.allclose(plan.query("tri_area"), oc.areas(), rtol=1e-13)
+    # indexing is bit-exact: same hinge enumeration, same stencils
+    assert np.array_equal(plan.query("hinge_verts").reshape(-1, 4), oc.hinges())
+    assert np.allclose(plan.query("hinge_K").reshape(-1, 4), oc.hinge_rows(), rtol=1e-11, atol=1e-13)
+    w, r = oc.hinge_weights()
+    wr = plan.query("hinge_wr").reshape(-1, 2)
+    assert np.allclose(wr[:, 0], w, rtol=1e-12) and np.allclose(wr[:, 1], r, rtol=1e-10, atol=1e-13)
+    A = plan.query("system").reshape(n, n)
+    assert np.allclose(A, oc.system_matrix(), rtol=1e-11, atol=1e-12)
+    # D_m^-1 against the oracle's G = D_m^-T [[-1,1,0],[-1,0,1]]
+    dm = plan.query("tri_dminv").reshape(T, 3)
+    G = oc.G()
+    assert np.allclose(G[:, 0, 1], dm[:, 0], rtol=1e-12)
+    assert np.allclose(G[:, 1, 1], dm[:, 1], rtol=1e-10, atol=1e-13)
+    assert np.allclose(G[:, 1, 2], dm[:, 2], rtol=1e-12)
+
+
+def test_internal_ordering_is_a_permutation_and_stays_internal(cell):
+    rest, tris, mat, plan, oc = cell
+    perm = plan.query("perm")
+    assert sorted(perm.tolist()) == list(range(rest.shape[0]))
+
+
+def test_operator_is_the_inverse_up_to_the_drop_rule(cell):
+    rest, tris, mat, plan, oc = cell
+    n = rest.shape[0]
+    A = oc.system_matrix()
+    Tinv = np.linalg.inv(A)
+    op = plan.query("operator").reshape(n, n)
+    tol = plan.info()["inv_drop_tol"]
+    assert tol == pytest.approx(2.0 ** -24)
+    kept = op != 0
+    assert np.array_equal(kept, kept.T)                                 # symmetric pattern
+    assert np.allclose(op[kept], Tinv[kept], rtol=3e-7, atol=0)         # fp32 rounding of kept entries
+    dropped_l1 = np.abs(np.where(kept, 0.0, Tinv)).sum(axis=1)
+    assert (dropped_l1 <= tol * np.abs(Tinv).sum(axis=1) * (1 + 1e-9)).all()
+    # the operator applied to A_sys is the identity to fp32 accuracy
+    assert np.abs(op @ A - np.eye(n)).max() < 5e-6
+    dense = NpfemPlan(tris, rest, mat, DT, inv_drop_tol=0.0)
+    opd = dense.query("operator").reshape(n, n)
+    assert np.allclose(opd, Tinv, rtol=3e-7, atol=1e-12)
+    assert dense.info()["n_op_blocks"] == dense.info()["n_vblocks"] ** 2
+
+
+def test_increment_form_with_the_kept_operator_reproduces_oracle_iterates():
+    """The algebra of the kernel, d <- d + T (f_int(s + d) - (m/h^2) d), evaluated in fp64 with
+    the plan's (dropped, fp32-rounded) operator, against the oracle's absolute-form iterates."""
+    rest, tris = W.rest_shape("rbc", 2)
+    mat = W.default_material(rest, tris)
+    plan, oc = NpfemPlan(tris, rest, mat, DT), O.OracleCell(tris, rest, mat, DT)
+    n = rest.shape[0]
+    op = plan.query("operator").reshape(n, n)
+    m = oc.masses()[:, None]
+    rng = np.random.default_rng(5)
+    x0 = rest + 50.0
+    v0 = rng.standard_normal((n, 3)) * 1e-3
+    f = rng.standard_normal((n, 3)) * 1e-3
+    _, _, iterates, _ = oc.step_cell(x0, v0, f, 6, trace=True)
+    s = x0 + DT * v0 + DT * DT * f / m
+    d = np.zeros((n, 3))
+    for k in range(6):
+        e = oc.fint(s + d)
+        d = d + op @ (e - m / DT ** 2 * d)
+        err = np.abs((s + d) - iterates[k + 1]).max()
+        motion = np.abs(iterates[k + 1] - x0).max()
+        assert err <= 2e-6 * motion, (k, err, motion)
+
+
+def test_argument_errors_are_codes_not_crashes():
+    rest, tris = W.rest_shape("rbc", 1)
+    mat = W.default_material(rest, tris)
+    NpfemPlan(tris, rest, mat, DT)
+    bad = dict(mat, c_alpha=0.1)
+    with pytest.raises(NpfemError) as e:
+        NpfemPlan(tris, rest, bad, DT)
+    assert e.value.code == -1 and "damping" in str(e.value)
+    with pytest.raises(NpfemError):
+        NpfemPlan(tris, rest, dict(mat, s_min=1.2, s_max=1.0), DT)
+    with pytest.raises(NpfemError):
+        NpfemPlan(tris, rest, mat, 0.0)
+    with pytest.raises(NpfemError):
+        NpfemPlan(tris[:-1], rest, mat, DT)                              # open mesh
+    flipped = tris.copy()
+    flipped[3] = flipped[3][[0, 2, 1]]
+    with pytest.raises(NpfemError):
+        NpfemPlan(flipped, rest, mat, DT)                                # inconsistent orientation
+    with pytest.raises(NpfemError):
+        NpfemPlan(tris[:, [0, 2, 1]], rest, mat, DT)                     # inward: V0 < 0
+    big_rest, big_tris = W.rest_shape("rbc", 4)
+    with pytest.raises(NpfemError) as e:
+        NpfemPlan(big_tris, big_rest, W.default_material(big_rest, big_tris), DT)
+    assert e.value.code == -4
+    with pytest.raises(NpfemError):
+        NpfemPlan(tris, rest, mat, DT, cells_per_cta=9)
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful on a box without CUDA")
+def test_no_cpu_fallback_create_fails_loudly_without_cuda():
+    rest, tris = W.rest_shape("rbc", 1)
+    with pytest.raises(NpfemError) as e:
+        NpfemHandle(tris, rest, W.default_material(rest, tris), DT)
+    assert e.value.code == -3

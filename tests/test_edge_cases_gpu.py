@@ -1,0 +1,187 @@
+"""GPU edge cases of the C ABI: empty and ragged inputs, strides, option variants, clamp bands,
+degenerate iteration counts, the host-buffer entry point and run-to-run determinism."""
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from oracle import npfem_oracle as O
+from paper_2011_04332_b200 import NpfemError, NpfemHandle
+from paper_2011_04332_b200.harness import DeviceGroup, from_strided, to_strided
+from tests.parity_util import gpu_trajectory, max_abs_err, oracle_trajectory, position_tolerance
+
+pytestmark = pytest.mark.gpu
+
+
+def _small_workload(kind="rbc", level=2, n_cells=7, seed=7, sigma=1e-3, box=100.0, **mat_over):
+    rest, tris = W.rest_shape(kind, level)
+    mat = W.default_material(rest, tris, **mat_over)
+    rng = np.random.Generator(np.random.PCG64([seed, 1]))
+    rot, trans = W.random_rigid_placements(n_cells, box, 5.0, rng)
+    pos0 = W.place_cells(rest, rot, trans)
+    vel0 = (rng.standard_normal(pos0.shape) * 1e-4).astype(np.float32)
+    forces = [W.gaussian_forces(pos0.shape, sigma, seed, s) for s in range(3)]
+    return rest, tris, mat, pos0, vel0, forces
+
+
+class _G:        # minimal stand-in for workloads.CellGroup
+    def __init__(self, rest, tris, mat, pos0, vel0):
+        self.rest, self.tris, self.material, self.pos0, self.vel0 = rest, tris, mat, pos0, vel0
+        self.diameter = W.shapes.cell_diameter(rest)
+
+
+def _parity(g, forces, n_iters, dt=0.1, **options):
+    tol = position_tolerance(g)
+    worst = 0.0
+    for (po, vo), (pg, vg) in zip(oracle_trajectory(g, dt, forces, n_iters),
+                                  gpu_trajectory(g, dt, forces, n_iters, **options)):
+        err = max_abs_err(pg, po)
+        worst = max(worst, err)
+        assert err <= tol
+        scale = np.abs(vo).max() * dt
+        assert np.abs(vg.astype(np.float64) - vo).max() * dt <= 2e-3 * scale + 0.02 * err
+    return worst
+
+
+def test_zero_cells_is_a_no_op_and_null_pointers_are_rejected():
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=1)
+    h = NpfemHandle(tris, rest, mat, 0.1)
+    h.step(0, None, None, None, 5)                       # n_cells == 0: nothing to do, no error
+    with pytest.raises(NpfemError):
+        h.step(1, None, None, None, 5)
+    p = to_strided(pos0, h.cell_stride)
+    with pytest.raises(NpfemError):
+        h.step(-1, p, p, p, 5)
+    with pytest.raises(NpfemError):
+        h.step(1, p, p, p, -1)
+
+
+def test_n_iters_zero_is_the_inertial_prediction():
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=3)
+    g = _G(rest, tris, mat, pos0, vel0)
+    (pg, vg), = list(gpu_trajectory(g, 0.1, forces[:1], 0))
+    oc = O.OracleCell(tris, rest, mat, 0.1)
+    m = oc.masses()[None, :, None]
+    inc = 0.1 * vel0.astype(np.float64) + 0.01 * forces[0].astype(np.float64) / m
+    assert np.abs(vg * 0.1 - inc).max() <= 1e-6 * np.abs(inc).max()
+    assert max_abs_err(pg, pos0.astype(np.float64) + inc) <= 1e-5
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_cells_per_cta_variants_and_ragged_tails(k):
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=7)
+    _parity(_G(rest, tris, mat, pos0, vel0), forces, 6, cells_per_cta=k)
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_global_step_modes_simt_and_3xtf32(mode):
+    rest, tris, mat, pos0, vel0, forces = _small_workload(level=3, n_cells=6)
+    _parity(_G(rest, tris, mat, pos0, vel0), forces, 8, global_mode=mode)
+
+
+def test_dense_operator_matches_dropped_operator():
+    """inv_drop_tol = 0 keeps every entry of A_sys^-1; the default drop rule must agree with it
+    far inside the parity tolerance."""
+    rest, tris, mat, pos0, vel0, forces = _small_workload(level=3, n_cells=5)
+    g = _G(rest, tris, mat, pos0, vel0)
+    a = list(gpu_trajectory(g, 0.1, forces, 10, inv_drop_tol=0.0))
+    b = list(gpu_trajectory(g, 0.1, forces, 10))
+    for (pa, va), (pb, vb) in zip(a, b):
+        assert np.abs(va - vb).max() * 0.1 <= 1e-5 * np.abs(va).max() * 0.1 + 1e-9
+    _parity(g, forces, 10, inv_drop_tol=0.0)
+
+
+def test_platelets_pack_many_cells():
+    rest, tris, mat, pos0, vel0, forces = _small_workload(kind="plt", level=1, n_cells=41)
+    _parity(_G(rest, tris, mat, pos0, vel0), forces, 20)
+
+
+@pytest.mark.parametrize("stride_extra", [0, 1, 2, 64])
+def test_custom_cell_strides_and_padding_is_preserved(stride_extra):
+    """3*n floats = 8 (mod 16) bytes for every icosphere: stride 3n puts odd cells off 16-byte
+    alignment; padding floats must come back untouched."""
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=5)
+    n = rest.shape[0]
+    stride = 3 * n + stride_extra
+    h = NpfemHandle(tris, rest, mat, 0.1, stride, 5)
+    assert h.cell_stride == stride
+    pos, vel = to_strided(pos0, stride), to_strided(vel0, stride)
+    fx = to_strided(forces[0], stride)
+    pos[:, 3 * n:] = 123.0
+    vel[:, 3 * n:] = -7.0
+    h.step(5, pos, vel, fx, 10)
+    torch.cuda.synchronize()
+    assert (pos[:, 3 * n:] == 123.0).all() and (vel[:, 3 * n:] == -7.0).all()
+    oc = O.OracleCell(tris, rest, mat, 0.1)
+    po, vo = oc.step(pos0, vel0, forces[0], 10)
+    assert max_abs_err(from_strided(pos, n), po) <= 1e-4 * 8.0
+    assert np.abs(from_strided(vel, n) - vo).max() <= 2e-3 * np.abs(vo).max()
+    with pytest.raises(NpfemError):
+        NpfemHandle(tris, rest, mat, 0.1, 3 * n - 1, 5)
+
+
+def test_nontrivial_clamp_bands_under_large_forces():
+    """Strain band [0.9, 1.1], area band [0.95, 1.05], volume band [0.99, 1.01]: forces large
+    enough that some elements sit inside, some outside their bands (exercises every clamp
+    branch and the hyperbola projection)."""
+    rest, tris, mat, pos0, vel0, forces = _small_workload(
+        n_cells=4, sigma=2e-2, s_min=0.9, s_max=1.1, a_min=0.95, a_max=1.05, v_min=0.99,
+        v_max=1.01)
+    g = _G(rest, tris, mat, pos0, vel0)
+    forces = [f for f in forces] * 4                     # 12 steps
+    _parity(g, forces, 10)
+    # the bands were really active / inactive on different elements
+    oc = O.OracleCell(tris, rest, mat, 0.1)
+    last = list(oracle_trajectory(g, 0.1, forces, 10))[-1][0][0]
+    sv = np.array([np.linalg.svd(oc.deformation_gradient(t, last), compute_uv=False)
+                   for t in range(tris.shape[0])])
+    assert (sv.max(axis=1) > 1.1).any() or (sv.min(axis=1) < 0.9).any()
+    assert ((sv > 0.9) & (sv < 1.1)).all(axis=1).any()
+
+
+def test_shrunk_and_inflated_cells_exercise_volume_and_area_projection():
+    """Start from uniformly scaled rest shapes (0.9x and 1.15x): large volume/area violations."""
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=2, sigma=1e-3)
+    c = pos0.mean(axis=1, keepdims=True)
+    pos0 = (c + (pos0 - c) * np.array([0.9, 1.15], dtype=np.float32)[:, None, None]).astype(np.float32)
+    g = _G(rest, tris, mat, pos0, np.zeros_like(pos0))
+    _parity(g, forces * 3, 10)
+
+
+def test_step_host_matches_device_step_bit_for_bit_and_is_deterministic():
+    rest, tris, mat, pos0, vel0, forces = _small_workload(level=3, n_cells=23)
+    n = rest.shape[0]
+    h = NpfemHandle(tris, rest, mat, 0.1)
+    stride = h.cell_stride
+    runs = []
+    for _ in range(2):
+        pos, vel, fx = (to_strided(a, stride) for a in (pos0, vel0, forces[0]))
+        h.step(23, pos, vel, fx, 10)
+        torch.cuda.synchronize()
+        runs.append((pos.cpu().numpy().copy(), vel.cpu().numpy().copy()))
+    assert np.array_equal(runs[0][0], runs[1][0]) and np.array_equal(runs[0][1], runs[1][1])
+    hp = [to_strided(a, stride, device="cpu").pin_memory() for a in (pos0, vel0, forces[0])]
+    h.step_host(23, hp[0], hp[1], hp[2], 10)
+    assert np.array_equal(hp[0].numpy(), runs[0][0]) and np.array_equal(hp[1].numpy(), runs[0][1])
+
+
+def test_step_on_a_side_stream():
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=5)
+    dg = DeviceGroup(tris, rest, mat, 0.1, pos0, vel0)
+    dg.set_forces(forces[0])
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        dg.step(10, stream=st)
+    st.synchronize()
+    pg, vg = dg.state()
+    oc = O.OracleCell(tris, rest, mat, 0.1)
+    po, vo = oc.step(pos0, vel0, forces[0], 10)
+    assert max_abs_err(pg, po) <= 8e-4
+
+
+def test_mesh_too_large_for_one_cta_is_rejected_loudly():
+    rest, tris = W.rest_shape("rbc", 4)                  # 2562 vertices > 1024
+    with pytest.raises(NpfemError) as e:
+        NpfemHandle(tris, rest, W.default_material(rest, tris), 0.1)
+    assert e.value.code == -4
