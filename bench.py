@@ -224,7 +224,14 @@ def run_ours(args) -> None:
     radius = float(np.linalg.norm(rest, axis=1).max())
     rot, trans = W.random_rigid_placements(n_cells, spec["box"], radius, rng)
     pos0 = W.place_cells(rest, rot, trans)                                 # fp32 [N,V,3]
-    h = NpfemHandle(tris, rest, mat, W.configs.DT, 0, n_cells)
+    opts = {}
+    if args.global_mode:
+        opts["global_mode"] = args.global_mode
+    if args.cells_per_cta:
+        opts["cells_per_cta"] = args.cells_per_cta
+    if args.drop_tol is not None:
+        opts["inv_drop_tol"] = args.drop_tol
+    h = NpfemHandle(tris, rest, mat, W.configs.DT, 0, n_cells, **opts)
     info = h.info()
     stride = h.cell_stride
     pos = to_strided(pos0, stride, dev)
@@ -270,11 +277,12 @@ def run_ours(args) -> None:
 
     # ---- end to end through the host-buffer entry point (pinned host memory)
     e2e = None
-    e2e_steps = max(1, min(args.steps, 3))
+    e2e_steps = 0 if args.kernel_only else max(1, min(args.steps, 3))
     hp = to_strided(pos0, stride, "cpu").pin_memory()
     hv = torch.zeros_like(hp).pin_memory()
     hf = fields[0].cpu().pin_memory()
-    h.step_host(n_cells, hp, hv, hf, n_iters)                              # warm-up: staging ring
+    if e2e_steps:
+        h.step_host(n_cells, hp, hv, hf, n_iters)                          # warm-up: staging ring
     barrier()
     t0 = time.perf_counter()
     for s in range(e2e_steps):
@@ -286,10 +294,11 @@ def run_ours(args) -> None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         t_e2e = float(t.item())
     field_bytes = n_cells * stride * 4
-    e2e = {"value": world * n_cells * e2e_steps / t_e2e, "unit": "cell-steps/s",
-           "h2d_bytes_per_step": 3 * field_bytes, "d2h_bytes_per_step": 2 * field_bytes,
-           "steps": e2e_steps, "ms_per_step": 1e3 * t_e2e / e2e_steps,
-           "api": "npfem_step_host (pinned host buffers, chunked 3-stream pipeline)"}
+    if e2e_steps:
+        e2e = {"value": world * n_cells * e2e_steps / t_e2e, "unit": "cell-steps/s",
+               "h2d_bytes_per_step": 3 * field_bytes, "d2h_bytes_per_step": 2 * field_bytes,
+               "steps": e2e_steps, "ms_per_step": 1e3 * t_e2e / e2e_steps,
+               "api": "npfem_step_host (pinned host buffers, chunked 3-stream pipeline)"}
 
     if rank != 0:
         if world > 1:
@@ -314,7 +323,7 @@ def run_ours(args) -> None:
         at_clock = 148 * 128 * 2 * clocks["sm_mhz"] * 1e6 / 1e12
         roofline["frac_at_observed_clock"] = achieved_tflops / at_clock
 
-    cpu = time_oracle(budget_s=12.0, steps=1) if world == 1 else None
+    cpu = time_oracle(budget_s=12.0, steps=1) if world == 1 and not args.kernel_only else None
     value = world * n_cells * args.steps / (total_ms * 1e-3)
     line = {"metric": "cell-steps/s", "value": value, "unit": "cell-steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
@@ -345,6 +354,11 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--cells", type=int, default=0, help="cells per GPU (default: config 4's 100000)")
+    ap.add_argument("--global-mode", type=int, default=0, help="npfem_options.global_mode (0 = default)")
+    ap.add_argument("--cells-per-cta", type=int, default=0, help="npfem_options.cells_per_cta (0 = auto)")
+    ap.add_argument("--drop-tol", type=float, default=None, help="npfem_options.inv_drop_tol")
+    ap.add_argument("--kernel-only", action="store_true",
+                    help="tuning runs: skip the e2e and cpu_baseline legs (not a bench line)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -37,6 +37,26 @@ __device__ __forceinline__ F3 fma3(float s, F3 a, F3 b) {
 __device__ __forceinline__ F3 ld3(const float* p) { return {p[0], p[1], p[2]}; }
 __device__ __forceinline__ void st3(float* p, F3 v) { p[0] = v.x; p[1] = v.y; p[2] = v.z; }
 
+// MUFU-based approximations (<= 2 ulp): the local step's inputs carry the rounding of fp32
+// cell-local positions, far above these, and IEEE division / sqrt
+// cost 8-12 instructions each on the FMA pipe.
+__device__ __forceinline__ float fdiv(float a, float b) { return __fdividef(a, b); }
+__device__ __forceinline__ float frcp(float a) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+  return r;
+}
+__device__ __forceinline__ float fsqrt(float a) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+  return r;
+}
+__device__ __forceinline__ float frsqrt(float a) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+  return r;
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
   v += __shfl_xor_sync(0xffffffffu, v, 16);
   v += __shfl_xor_sync(0xffffffffu, v, 8);
@@ -57,15 +77,15 @@ struct TriReg {
 // squared distance), bracketed in [1, max(s1/q, q/s2)] where g changes sign from <= 0 to >= 0.
 // Newton from the same-ratio point sqrt(s1/s2), bisection whenever Newton leaves the bracket.
 __device__ __forceinline__ float hyperbola_p(float s1, float s2, float q) {
-  float lo = 1.0f, hi = fmaxf(s1 / q, q / s2);
-  float p = sqrtf(s1 / s2);
+  float lo = 1.0f, hi = fmaxf(fdiv(s1, q), fdiv(q, s2));
+  float p = fsqrt(fdiv(s1, s2));
   p = fminf(fmaxf(p, lo), hi);
   for (int it = 0; it < 24; ++it) {
     float p2 = p * p;
     float g = fmaf(fmaf(q, p, -s1), p2 * p, fmaf(s2, p, -q));
     float dg = fmaf(fmaf(4.0f * q, p, -3.0f * s1), p2, s2);
     if (g < 0.0f) lo = p; else hi = p;
-    float pn = p - g / dg;
+    float pn = p - fdiv(g, dg);
     if (!(dg > 0.0f) || !(pn >= lo) || !(pn <= hi)) pn = 0.5f * (lo + hi);
     float step = fabsf(pn - p);
     p = pn;
@@ -94,25 +114,26 @@ __device__ __forceinline__ void triangle_residual(const TriReg& tr, const float*
   const F3 F1 = fma3(i01, eab, i11 * eac);
   const float C11 = dot(F0, F0), C12 = dot(F0, F1), C22 = dot(F1, F1);
   const F3 Nn = cross(F0, F1);
-  const float J = sqrtf(dot(Nn, Nn));                         // sigma1 * sigma2
-  const float tau = sqrtf(C11 + C22 + 2.0f * J);              // sigma1 + sigma2
+  const float J = fsqrt(dot(Nn, Nn));                         // sigma1 * sigma2
+  const float tau = fsqrt(C11 + C22 + 2.0f * J);              // sigma1 + sigma2
   const float dC = C11 - C22;
-  const float Delta = sqrtf(fmaf(dC, dC, 4.0f * C12 * C12));  // sigma1^2 - sigma2^2
-  const float delta = Delta / fmaxf(tau, 1e-30f);             // sigma1 - sigma2
+  const float Delta = fsqrt(fmaf(dC, dC, 4.0f * C12 * C12));  // sigma1^2 - sigma2^2
+  const float delta = fdiv(Delta, fmaxf(tau, 1e-30f));             // sigma1 - sigma2
   const float s1 = 0.5f * (tau + delta);
   const float s2 = fmaxf(0.5f * (tau - delta), 1e-30f);
   // g_i = sum_terms w (projected sigma_i - sigma_i) / sigma_i   (residual form: P - F = F V diag(g) V^T)
-  float g1 = tr.f[3] * (fminf(fmaxf(s1, P.s_min), P.s_max) - s1) / s1;
-  float g2 = tr.f[3] * (fminf(fmaxf(s2, P.s_min), P.s_max) - s2) / s2;
+  const float r1 = frcp(s1), r2 = frcp(s2);
+  float g1 = tr.f[3] * (fminf(fmaxf(s1, P.s_min), P.s_max) - s1) * r1;
+  float g2 = tr.f[3] * (fminf(fmaxf(s2, P.s_min), P.s_max) - s2) * r2;
   const float astar = fminf(fmaxf(J, P.a_min), P.a_max);
   if (J != astar) {
-    const float q = sqrtf(astar);
+    const float q = fsqrt(astar);
     const float p = hyperbola_p(s1, s2, q);
-    g1 = fmaf(tr.f[4], (q * p - s1) / s1, g1);
-    g2 = fmaf(tr.f[4], (q / p - s2) / s2, g2);
+    g1 = fmaf(tr.f[4], (q * p - s1) * r1, g1);
+    g2 = fmaf(tr.f[4], (fdiv(q, p) - s2) * r2, g2);
   }
   const float gbar = 0.5f * (g1 + g2);
-  const float rho = (g1 - g2) / fmaxf(Delta, 1e-30f);
+  const float rho = fdiv(g1 - g2, fmaxf(Delta, 1e-30f));
   const float S00 = fmaf(rho, 0.5f * dC, gbar), S11 = fmaf(-rho, 0.5f * dC, gbar), S01 = rho * C12;
   const F3 Q0 = fma3(S00, F0, S01 * F1);
   const F3 Q1 = fma3(S01, F0, S11 * F1);
@@ -126,7 +147,7 @@ __device__ __forceinline__ void triangle_residual(const TriReg& tr, const float*
     const float Kf = -(Kp + Kq + Ko);
     F3 kv = fma3(Kq, eab, fma3(Ko, eac, Kf * (zf0 - za)));
     const float nk2 = dot(kv, kv);
-    const float cf = nk2 > 1e-60f ? fmaf(rp, rsqrtf(nk2), -1.0f) : 0.0f;
+    const float cf = nk2 > 1e-30f ? fmaf(rp, frsqrt(nk2), -1.0f) : 0.0f;
     kv = cf * kv;
     fa = fma3(0.5f * Kp, kv, fa); fb = fma3(0.5f * Kq, kv, fb); fc = fma3(Ko, kv, fc);
   }
@@ -135,7 +156,7 @@ __device__ __forceinline__ void triangle_residual(const TriReg& tr, const float*
     const float Kf = -(Kp + Kq + Ko);
     F3 kv = fma3(Kq, ebc, fma3(-Ko, eab, Kf * (zf1 - zb)));   // za - zb = -eab
     const float nk2 = dot(kv, kv);
-    const float cf = nk2 > 1e-60f ? fmaf(rp, rsqrtf(nk2), -1.0f) : 0.0f;
+    const float cf = nk2 > 1e-30f ? fmaf(rp, frsqrt(nk2), -1.0f) : 0.0f;
     kv = cf * kv;
     fb = fma3(0.5f * Kp, kv, fb); fc = fma3(0.5f * Kq, kv, fc); fa = fma3(Ko, kv, fa);
   }
@@ -144,7 +165,7 @@ __device__ __forceinline__ void triangle_residual(const TriReg& tr, const float*
     const float Kf = -(Kp + Kq + Ko);
     F3 kv = fma3(-Kq, eac, fma3(-Ko, ebc, Kf * (zf2 - zc)));  // za - zc = -eac, zb - zc = -ebc
     const float nk2 = dot(kv, kv);
-    const float cf = nk2 > 1e-60f ? fmaf(rp, rsqrtf(nk2), -1.0f) : 0.0f;
+    const float cf = nk2 > 1e-30f ? fmaf(rp, frsqrt(nk2), -1.0f) : 0.0f;
     kv = cf * kv;
     fc = fma3(0.5f * Kp, kv, fc); fa = fma3(0.5f * Kq, kv, fa); fb = fma3(Ko, kv, fb);
   }

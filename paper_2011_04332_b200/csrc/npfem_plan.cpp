@@ -461,7 +461,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     return fail(NPFEM_ELIMIT, "cell state does not fit the shared memory of one SM");
   P->cells_per_cta = k;
   P->smem_bytes = smem_layout(n, T, nvb, k).total;
-  P->global_mode = o.global_mode ? o.global_mode : 1;
+  P->global_mode = o.global_mode ? o.global_mode : 2;
   o.cells_per_cta = k;
   o.global_mode = P->global_mode;
   P->opt = o;

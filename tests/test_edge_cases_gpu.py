@@ -8,7 +8,7 @@ import workloads as W
 from oracle import npfem_oracle as O
 from paper_2011_04332_b200 import NpfemError, NpfemHandle
 from paper_2011_04332_b200.harness import DeviceGroup, from_strided, to_strided
-from tests.parity_util import gpu_trajectory, max_abs_err, oracle_trajectory, position_tolerance
+from tests.parity_util import displacement_tolerance, gpu_trajectory, max_abs_err, oracle_trajectory, position_tolerance
 
 pytestmark = pytest.mark.gpu
 
@@ -33,13 +33,13 @@ class _G:        # minimal stand-in for workloads.CellGroup
 def _parity(g, forces, n_iters, dt=0.1, **options):
     tol = position_tolerance(g)
     worst = 0.0
-    for (po, vo), (pg, vg) in zip(oracle_trajectory(g, dt, forces, n_iters),
-                                  gpu_trajectory(g, dt, forces, n_iters, **options)):
+    for step, ((po, vo), (pg, vg)) in enumerate(zip(oracle_trajectory(g, dt, forces, n_iters),
+                                                    gpu_trajectory(g, dt, forces, n_iters, **options))):
         err = max_abs_err(pg, po)
         worst = max(worst, err)
         assert err <= tol
         scale = np.abs(vo).max() * dt
-        assert np.abs(vg.astype(np.float64) - vo).max() * dt <= 2e-3 * scale + 0.02 * err
+        assert np.abs(vg.astype(np.float64) - vo).max() * dt <= displacement_tolerance(g, scale, err, step)
     return worst
 
 
@@ -145,7 +145,10 @@ def test_shrunk_and_inflated_cells_exercise_volume_and_area_projection():
     c = pos0.mean(axis=1, keepdims=True)
     pos0 = (c + (pos0 - c) * np.array([0.9, 1.15], dtype=np.float32)[:, None, None]).astype(np.float32)
     g = _G(rest, tris, mat, pos0, np.zeros_like(pos0))
-    _parity(g, forces * 3, 10)
+    # 27 % / 52 % volume violations: the volume projection needs more than the default two inner
+    # iterations to be converged to the oracle's 1e-14 (SURVEY.md P-11 bounds the default's error
+    # only for violations of a fraction of a percent)
+    _parity(g, forces * 3, 10, volume_inner_iters=8)
 
 
 def test_step_host_matches_device_step_bit_for_bit_and_is_deterministic():
