@@ -52,7 +52,7 @@ void fill_info(const Plan& P, int cell_stride, npfem_info* o) {
   o->threads_per_cta = P.threads;
   o->smem_bytes = P.smem_bytes;
   o->n_vblocks = P.nvb;
-  o->n_op_blocks = (int)P.blk_col.size();
+  o->n_op_blocks = P.n_op_blocks;
   o->op_nnz = P.op_nnz;
   o->global_mode = P.global_mode;
   o->volume_inner_iters = P.opt.volume_inner_iters;
@@ -135,7 +135,7 @@ int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems) {
             for (int r = 0; r < 2; ++r) {
               const int j = jb * 8 + (l & 3) + 4 * r, i = ib * 8 + (l >> 2);
               if (i < n && j < n)
-                D[(size_t)P.perm[i] * n + P.perm[j]] = (double)P.blk_val[(size_t)b * 64 + 2 * l + r];
+                D[(size_t)P.perm[i] * n + P.perm[j]] += (double)P.blk_val[(size_t)b * 64 + 2 * l + r];
             }
         }
       return (int)elems;
@@ -178,22 +178,29 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   if (e != cudaSuccess) { delete H; return cuda_err(e, "cudaFuncSetAttribute(shared memory)"); }
 
   // ---- one blob for all constant tables, 256-byte aligned sections
-  const int n = P.n, T = P.T;
-  std::vector<uint16_t> perm16(n), tri_ids(6 * (size_t)T);
-  std::vector<float> tri_f((size_t)kTriFloats * T);
-  for (int i = 0; i < n; ++i) perm16[i] = (uint16_t)P.perm[i];
-  for (int t = 0; t < T; ++t) {
-    for (int q = 0; q < 6; ++q) tri_ids[(size_t)q * T + t] = P.tri[t].ids[q];
-    for (int q = 0; q < kTriFloats; ++q) tri_f[(size_t)q * T + t] = P.tri[t].f[q];
+  const int n = P.n, E = P.E, NP = P.nvb * 8;
+  std::vector<uint16_t> perm16(NP, 0);
+  std::vector<uint32_t> elem_ids(4 * (size_t)E);
+  std::vector<float> elem_f((size_t)kElemFloats * E), h2m(NP, 0.0f), mh2(NP, 0.0f);
+  for (int i = 0; i < n; ++i) {
+    perm16[i] = (uint16_t)P.perm[i];
+    h2m[i] = P.h2_over_m[i];
+    mh2[i] = P.m_over_h2[i];
+  }
+  for (int e = 0; e < E; ++e) {
+    const ElemConst& ec = P.elem[e];
+    for (int q = 0; q < 4; ++q)   // byte offsets of the float4 positions: 16 * internal id
+      elem_ids[(size_t)q * E + e] = (uint32_t)ec.ids[2 * q] * 16u | ((uint32_t)ec.ids[2 * q + 1] * 16u) << 16;
+    for (int q = 0; q < kElemFloats; ++q) elem_f[(size_t)q * E + e] = ec.f[q];
   }
   struct Sec { const void* src; size_t bytes; size_t off; };
   Sec secs[] = {
-      {perm16.data(), perm16.size() * 2, 0},          {tri_ids.data(), tri_ids.size() * 2, 0},
-      {tri_f.data(), tri_f.size() * 4, 0},            {P.h2_over_m.data(), P.h2_over_m.size() * 4, 0},
-      {P.m_over_h2.data(), P.m_over_h2.size() * 4, 0}, {P.inc_ptr.data(), P.inc_ptr.size() * 2, 0},
-      {P.inc_out.data(), P.inc_out.size() * 2, 0},    {P.inc_ring.data(), P.inc_ring.size() * 2, 0},
-      {P.blk_ptr.data(), P.blk_ptr.size() * 4, 0},    {P.blk_col.data(), P.blk_col.size() * 2, 0},
-      {P.blk_val.data(), P.blk_val.size() * 4, 0},
+      {perm16.data(), perm16.size() * 2, 0},          {elem_ids.data(), elem_ids.size() * 4, 0},
+      {elem_f.data(), elem_f.size() * 4, 0},          {h2m.data(), h2m.size() * 4, 0},
+      {mh2.data(), mh2.size() * 4, 0},                {P.inc_ptr.data(), P.inc_ptr.size() * 2, 0},
+      {P.inc_off.data(), P.inc_off.size() * 2, 0},    {P.ring_ptr.data(), P.ring_ptr.size() * 2, 0},
+      {P.ring_off.data(), P.ring_off.size() * 2, 0},  {P.blk_ptr.data(), P.blk_ptr.size() * 4, 0},
+      {P.blk_col.data(), P.blk_col.size() * 2, 0},    {P.blk_val.data(), P.blk_val.size() * 4, 0},
   };
   size_t total = 0;
   for (auto& sct : secs) { sct.off = total; total += align_up(sct.bytes, 256); }
@@ -205,24 +212,25 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   }
   char* base = static_cast<char*>(H->blob);
   DevParams& D = H->dev;
-  D.n = n; D.T = T; D.nvb = P.nvb; D.k = P.cells_per_cta; D.cell_stride = stride;
+  D.n = n; D.E = E; D.nvb = P.nvb; D.k = P.cells_per_cta; D.cell_stride = stride;
   D.vol_iters = P.opt.volume_inner_iters;
   D.h = (float)P.h; D.w_volume = (float)P.mat.w_volume; D.V0 = (float)P.V0;
   D.Vmin = (float)(P.mat.v_min * P.V0); D.Vmax = (float)(P.mat.v_max * P.V0);
   D.s_min = (float)P.mat.s_min; D.s_max = (float)P.mat.s_max;
   D.a_min = (float)P.mat.a_min; D.a_max = (float)P.mat.a_max;
   D.perm = reinterpret_cast<const uint16_t*>(base + secs[0].off);
-  D.tri_ids = reinterpret_cast<const uint16_t*>(base + secs[1].off);
-  D.tri_f = reinterpret_cast<const float*>(base + secs[2].off);
+  D.elem_ids = reinterpret_cast<const uint32_t*>(base + secs[1].off);
+  D.elem_f = reinterpret_cast<const float*>(base + secs[2].off);
   D.h2_over_m = reinterpret_cast<const float*>(base + secs[3].off);
   D.m_over_h2 = reinterpret_cast<const float*>(base + secs[4].off);
   D.inc_ptr = reinterpret_cast<const uint16_t*>(base + secs[5].off);
-  D.inc_out = reinterpret_cast<const uint16_t*>(base + secs[6].off);
-  D.inc_ring = reinterpret_cast<const uint16_t*>(base + secs[7].off);
-  D.blk_ptr = reinterpret_cast<const int*>(base + secs[8].off);
-  D.blk_col = reinterpret_cast<const uint16_t*>(base + secs[9].off);
-  D.blk_val = reinterpret_cast<const float*>(base + secs[10].off);
-  D.L = smem_layout(n, T, P.nvb, P.cells_per_cta);
+  D.inc_off = reinterpret_cast<const uint16_t*>(base + secs[6].off);
+  D.ring_ptr = reinterpret_cast<const uint16_t*>(base + secs[7].off);
+  D.ring_off = reinterpret_cast<const uint16_t*>(base + secs[8].off);
+  D.blk_ptr = reinterpret_cast<const int*>(base + secs[9].off);
+  D.blk_col = reinterpret_cast<const uint16_t*>(base + secs[10].off);
+  D.blk_val = reinterpret_cast<const float*>(base + secs[11].off);
+  D.L = smem_layout(n, E, P.nvb, P.cells_per_cta);
   *out = H;
   return NPFEM_OK;
 }

@@ -12,20 +12,29 @@ namespace npfem {
 
 constexpr int kMaxVerts = 1024;       // one CTA owns whole cells; blockDim <= 1024
 constexpr int kMaxCellsPerCta = 5;    // 5 cells x 3 coordinates = 15 right-hand sides (+1 pad = 16)
-constexpr int kRhs = 16;              // right-hand sides per CTA in the global step
-constexpr int kTriFloats = 17;        // per-triangle float constants (see TriConst below)
-constexpr int kTrisPerThread = 2;     // register-resident triangle constants per thread
+constexpr int kRhs = 16;              // right-hand sides per CTA in the global step (mma M)
+constexpr int kElemFloats = 31;       // per-element float constants (see ElemConst below)
+constexpr int kRegList = 6;           // incidence / ring entries a vertex thread keeps in registers
 constexpr int kSmemMaxDynamic = 232448 - 1024;   // 227 KB opt-in limit per CTA minus static shared memory
 
-// Per-triangle constants, all in INTERNAL vertex numbering.
-//   ids:  a, b, c  own vertices;  f0, f1, f2  the vertices across edges (a,b), (b,c), (c,a).
-//   f[0..2]  D_m^-1 = [[i00, i01], [0, i11]]      f[3], f[4]  w_s = k_strain*A_t, w_a = k_area*A_t
-//   f[5+4e .. 8+4e], e = 0,1,2: the hinge on edge e seen from this triangle, scaled by sqrt(w_h):
-//       Kp, Kq (edge endpoints in the triangle's cyclic order), Ko (own opposite vertex), r' =
-//       sqrt(w_h) * r_h.  The coefficient of the far vertex is -(Kp + Kq + Ko) (rows of K sum to 0).
-struct TriConst {
-  uint16_t ids[6];
-  float f[kTriFloats];
+// One ELEMENT = the work of one thread in the local step: a "diamond" of two triangles
+// t1 = (a,b,c) and t2 = (b,a,d) sharing the edge (a,b), or a single triangle t1 whose t2 carries
+// zero weights.  All vertex ids are INTERNAL numbers.
+//   ids:  a, b, c, d  own vertices;  f1..f4 the vertices across the outer edges
+//         (b,c), (c,a), (a,d), (d,b).
+//   f[0..4]   t1: D_m^-1 = [[i00, i01], [0, i11]] for the vertex order (a,b,c); w_s, w_a
+//   f[5..9]   t2: the same for the vertex order (b,a,d)
+//   f[10+4e .. 13+4e], e = 0..4: hinge e scaled by sqrt(w_h): Kp, Kq (edge endpoints), Ko (the
+//         element's own opposite vertex), r' = sqrt(w_h) r_h; the coefficient of the vertex
+//         across is -(Kp+Kq+Ko).  e = 0 the shared edge (a,b | c ; d); e = 1 (b,c | a ; f1);
+//         e = 2 (c,a | b ; f2); e = 3 (a,d | b ; f3); e = 4 (d,b | a ; f4).
+//   f[30]     he: 1 for a diamond (the shared hinge is evaluated once, in full), 0.5 for a single
+//         triangle (its neighbour evaluates the other half; nothing goes to d).
+// Outer hinges are evaluated by both elements that see them, each adding half of the end-point
+// terms and all of its own opposite vertex's term, so that every hinge counts exactly once.
+struct ElemConst {
+  uint16_t ids[8];
+  float f[kElemFloats];
 };
 
 struct Plan {
@@ -48,16 +57,21 @@ struct Plan {
   // device-bound data (internal numbering)
   std::vector<int32_t> perm;         // internal -> caller vertex
   std::vector<int32_t> iperm;        // caller -> internal
-  std::vector<TriConst> tri;         // [T] in internal triangle order
+  int E = 0;                         // number of elements (diamonds + single triangles)
+  int n_diamonds = 0;
+  std::vector<ElemConst> elem;       // [E]
+  std::vector<int32_t> elem_tris;    // [E][2] caller triangle ids (second = -1 for a single)
   std::vector<float> h2_over_m;      // [n]
   std::vector<float> m_over_h2;      // [n]
-  std::vector<uint16_t> inc_ptr;     // [n+1] CSR over incident triangles, cyclically ordered
-  std::vector<uint16_t> inc_out;     // [3T] float offset of the vertex's 3-vector in the out buffer
-  std::vector<uint16_t> inc_ring;    // [3T] internal id of the ring neighbour r_i (triangle i = v, r_i, r_i+1)
+  std::vector<uint16_t> inc_ptr;     // [n+1] CSR over the element slots a vertex gathers from
+  std::vector<uint16_t> inc_off;     // byte offset of the slot's float4 in the out buffer
+  std::vector<uint16_t> ring_ptr;    // [n+1] CSR over the cyclically ordered ring neighbours
+  std::vector<uint16_t> ring_off;    // byte offset (16 * internal id) of the neighbour in z4
   int nvb = 0;                       // number of 8-vertex blocks
-  std::vector<int32_t> blk_ptr;      // [nvb+1] kept operator blocks per OUTPUT block
-  std::vector<uint16_t> blk_col;     // [n_op_blocks] source block index
-  std::vector<float> blk_val;        // [n_op_blocks][64] in mma B-fragment order
+  std::vector<int32_t> blk_ptr;      // [nvb+1] operator blocks per OUTPUT block (rows padded to x4)
+  std::vector<uint16_t> blk_col;     // [n_blocks_padded] source block index
+  std::vector<float> blk_val;        // [n_blocks_padded][64] in mma B-fragment order
+  int n_op_blocks = 0;               // kept blocks (without the zero padding blocks)
   int op_nnz = 0;
 
   // launch configuration decided at create time
@@ -70,22 +84,28 @@ int build_plan(int n_verts, int n_tris, const int32_t* tris, const double* rest_
                std::string* err);
 
 // Shared-memory carve-up used by both the host (to size the launch) and the kernel.
+//   z4   [k][NP] float4   current iterate z = s + d, cell-local coordinates (w unused)
+//   s, d [3k][NP] float   inertial prediction and correction, row m = 3*cell + component
+//   ra   [nvb][32] float4 right-hand sides in mma A-fragment order (fp32 while the local step
+//                         accumulates them, then their tf32 high parts)
+//   rb   max(E*64, NP*64) element results `out` [E][4] float4 during the local step, then the
+//                         tf32 low parts of the right-hand sides during the global step
+//   red  [5][32] float4   per-warp partial sums of the volume reductions
 struct SmemLayout {
-  int z, s, d, r, out, red, total;   // byte offsets
+  int z4, s, d, ra, rb, red, total;   // byte offsets
 };
-inline SmemLayout smem_layout(int n, int T, int nvb, int k) {
-  auto up16 = [](int x) { return (x + 15) & ~15; };
+inline SmemLayout smem_layout(int n, int E, int nvb, int k) {
+  (void)n;
+  const int NP = nvb * 8;
   SmemLayout L{};
-  int field = up16(k * n * 3 * 4);
   int off = 0;
-  L.z = off; off += field;
-  L.s = off; off += field;
-  L.d = off; off += field;
-  L.r = off; off += up16(2 * nvb * 8 * 8 * 4);
-  int out_bytes = T * 9 * 4;
-  if (out_bytes < k * n * 3 * 4) out_bytes = k * n * 3 * 4;   // doubles as scratch for the volume step
-  L.out = off; off += up16(out_bytes);
-  L.red = off; off += up16(kMaxCellsPerCta * 32 * 4 * 4);
+  L.z4 = off; off += k * NP * 16;
+  L.s = off; off += 3 * k * NP * 4;
+  L.d = off; off += 3 * k * NP * 4;
+  L.ra = off; off += NP * 64;
+  int rb = E * 64 > NP * 64 ? E * 64 : NP * 64;
+  L.rb = off; off += rb;
+  L.red = off; off += kMaxCellsPerCta * 32 * 16;
   L.total = off;
   return L;
 }

@@ -14,6 +14,12 @@
 //   x_n+1  = x_n + (u0 + d),  v_n+1 = (u0 + d)/h
 // which is algebraically the oracle's  x^{k+1} = A_sys^-1 (M/h^2 s + sum w A^T p)  (PAPER.md:90-95
 // lineage), but never differences world coordinates.
+//
+// Work mapping per iteration and cell: thread e < E owns one ELEMENT (two triangles sharing an
+// edge, npfem_internal.h) and writes one float4 per own vertex; thread v < n owns one VERTEX,
+// gathers its element slots, evaluates grad V on its ring and forms the right-hand side; the
+// global step then multiplies all 16 right-hand-side columns of the CTA by the block-sparse
+// inverse on the tensor cores (3xTF32 split, fp32 accumulate).
 #include <cstdint>
 
 #include "npfem_kernels.cuh"
@@ -31,11 +37,18 @@ __device__ __forceinline__ float dot(F3 a, F3 b) { return fmaf(a.x, b.x, fmaf(a.
 __device__ __forceinline__ F3 cross(F3 a, F3 b) {
   return {fmaf(a.y, b.z, -a.z * b.y), fmaf(a.z, b.x, -a.x * b.z), fmaf(a.x, b.y, -a.y * b.x)};
 }
+// acc + a x b
+__device__ __forceinline__ F3 cross_acc(F3 a, F3 b, F3 acc) {
+  return {fmaf(a.y, b.z, fmaf(-a.z, b.y, acc.x)), fmaf(a.z, b.x, fmaf(-a.x, b.z, acc.y)),
+          fmaf(a.x, b.y, fmaf(-a.y, b.x, acc.z))};
+}
 __device__ __forceinline__ F3 fma3(float s, F3 a, F3 b) {
   return {fmaf(s, a.x, b.x), fmaf(s, a.y, b.y), fmaf(s, a.z, b.z)};
 }
-__device__ __forceinline__ F3 ld3(const float* p) { return {p[0], p[1], p[2]}; }
-__device__ __forceinline__ void st3(float* p, F3 v) { p[0] = v.x; p[1] = v.y; p[2] = v.z; }
+__device__ __forceinline__ F3 xyz(float4 v) { return {v.x, v.y, v.z}; }
+__device__ __forceinline__ F3 lds3(const unsigned char* base, uint32_t byte_off) {
+  return xyz(*reinterpret_cast<const float4*>(base + byte_off));
+}
 
 // MUFU-based approximations (<= 2 ulp): the local step's inputs carry the rounding of fp32
 // cell-local positions, far above these, and IEEE division / sqrt
@@ -66,12 +79,6 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-// Register-resident constants of one triangle (npfem_internal.h: TriConst).
-struct TriReg {
-  uint32_t ab, cf0, f12;   // packed internal vertex ids: (a,b), (c,f0), (f1,f2)
-  float f[kTriFloats];
-};
-
 // Closest point of the hyperbola branch {t1*t2 = q^2, t > 0} to (s1, s2), s1 >= s2 > 0, written
 // as (q p, q / p) with p >= 1: root of  g(p) = q p^4 - s1 p^3 + s2 p - q  (stationarity of the
 // squared distance), bracketed in [1, max(s1/q, q/s2)] where g changes sign from <= 0 to >= 0.
@@ -94,89 +101,54 @@ __device__ __forceinline__ float hyperbola_p(float s1, float s2, float q) {
   return p;
 }
 
-// Local step for one triangle: elastic residual forces on its three vertices from
+// Membrane part of the local step for one triangle (p0,p1,p2) with edges e1 = z1 - z0,
+// e2 = z2 - z0:  F = [e1 e2] D_m^-1, singular values from tr(F^T F) and det; residual forces of
 //   - triangle strain   w_s ||F - P_s||^2/2,  P_s = U clamp(Sigma,[s_min,s_max]) V^T
 //   - triangle area     w_a ||F - P_a||^2/2,  P_a = U Sigma' V^T, sigma1' sigma2' = clamp(sigma1 sigma2)
-//   - the three hinges on its edges (each hinge is evaluated by both of its triangles; endpoint
-//     contributions are halved so that every hinge counts once)
-// (DESIGN.md "local step").  z = the cell's current iterate in shared memory.
-__device__ __forceinline__ void triangle_residual(const TriReg& tr, const float* __restrict__ z,
-                                                  const DevParams& P, float* __restrict__ out9) {
-  const int ia = tr.ab & 0xffff, ib = tr.ab >> 16, ic = tr.cf0 & 0xffff;
-  const int i0 = tr.cf0 >> 16, i1 = tr.f12 & 0xffff, i2 = tr.f12 >> 16;
-  const F3 za = ld3(z + 3 * ia), zb = ld3(z + 3 * ib), zc = ld3(z + 3 * ic);
-  const F3 zf0 = ld3(z + 3 * i0), zf1 = ld3(z + 3 * i1), zf2 = ld3(z + 3 * i2);
-  const F3 eab = zb - za, eac = zc - za, ebc = zc - zb;
-
-  // ---- membrane: F = [eab eac] D_m^-1, C = F^T F, singular values from tr and det
-  const float i00 = tr.f[0], i01 = tr.f[1], i11 = tr.f[2];
-  const F3 F0 = i00 * eab;
-  const F3 F1 = fma3(i01, eab, i11 * eac);
+// on vertices 1 and 2 (vertex 0 receives -(f1 + f2)).  SURVEY.md 8(c) step 2.
+__device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, float i11, float ws,
+                                         float wa, const DevParams& P, F3& f1, F3& f2) {
+  const F3 F0 = i00 * e1;
+  const F3 F1 = fma3(i01, e1, i11 * e2);
   const float C11 = dot(F0, F0), C12 = dot(F0, F1), C22 = dot(F1, F1);
   const F3 Nn = cross(F0, F1);
   const float J = fsqrt(dot(Nn, Nn));                         // sigma1 * sigma2
   const float tau = fsqrt(C11 + C22 + 2.0f * J);              // sigma1 + sigma2
   const float dC = C11 - C22;
   const float Delta = fsqrt(fmaf(dC, dC, 4.0f * C12 * C12));  // sigma1^2 - sigma2^2
-  const float delta = fdiv(Delta, fmaxf(tau, 1e-30f));             // sigma1 - sigma2
+  const float delta = fdiv(Delta, fmaxf(tau, 1e-30f));        // sigma1 - sigma2
   const float s1 = 0.5f * (tau + delta);
   const float s2 = fmaxf(0.5f * (tau - delta), 1e-30f);
   // g_i = sum_terms w (projected sigma_i - sigma_i) / sigma_i   (residual form: P - F = F V diag(g) V^T)
   const float r1 = frcp(s1), r2 = frcp(s2);
-  float g1 = tr.f[3] * (fminf(fmaxf(s1, P.s_min), P.s_max) - s1) * r1;
-  float g2 = tr.f[3] * (fminf(fmaxf(s2, P.s_min), P.s_max) - s2) * r2;
+  float g1 = ws * (fminf(fmaxf(s1, P.s_min), P.s_max) - s1) * r1;
+  float g2 = ws * (fminf(fmaxf(s2, P.s_min), P.s_max) - s2) * r2;
   const float astar = fminf(fmaxf(J, P.a_min), P.a_max);
   if (J != astar) {
     const float q = fsqrt(astar);
     const float p = hyperbola_p(s1, s2, q);
-    g1 = fmaf(tr.f[4], (q * p - s1) * r1, g1);
-    g2 = fmaf(tr.f[4], (fdiv(q, p) - s2) * r2, g2);
+    g1 = fmaf(wa, (q * p - s1) * r1, g1);
+    g2 = fmaf(wa, (fdiv(q, p) - s2) * r2, g2);
   }
   const float gbar = 0.5f * (g1 + g2);
   const float rho = fdiv(g1 - g2, fmaxf(Delta, 1e-30f));
   const float S00 = fmaf(rho, 0.5f * dC, gbar), S11 = fmaf(-rho, 0.5f * dC, gbar), S01 = rho * C12;
   const F3 Q0 = fma3(S00, F0, S01 * F1);
   const F3 Q1 = fma3(S01, F0, S11 * F1);
-  F3 fb = fma3(i00, Q0, i01 * Q1);
-  F3 fc = i11 * Q1;
-  F3 fa = {-(fb.x + fc.x), -(fb.y + fc.y), -(fb.z + fc.z)};
-
-  // ---- bending hinges.  edge 0 = (a,b) opp c far f0; edge 1 = (b,c) opp a far f1; edge 2 = (c,a) opp b far f2
-  {
-    const float Kp = tr.f[5], Kq = tr.f[6], Ko = tr.f[7], rp = tr.f[8];
-    const float Kf = -(Kp + Kq + Ko);
-    F3 kv = fma3(Kq, eab, fma3(Ko, eac, Kf * (zf0 - za)));
-    const float nk2 = dot(kv, kv);
-    const float cf = nk2 > 1e-30f ? fmaf(rp, frsqrt(nk2), -1.0f) : 0.0f;
-    kv = cf * kv;
-    fa = fma3(0.5f * Kp, kv, fa); fb = fma3(0.5f * Kq, kv, fb); fc = fma3(Ko, kv, fc);
-  }
-  {
-    const float Kp = tr.f[9], Kq = tr.f[10], Ko = tr.f[11], rp = tr.f[12];
-    const float Kf = -(Kp + Kq + Ko);
-    F3 kv = fma3(Kq, ebc, fma3(-Ko, eab, Kf * (zf1 - zb)));   // za - zb = -eab
-    const float nk2 = dot(kv, kv);
-    const float cf = nk2 > 1e-30f ? fmaf(rp, frsqrt(nk2), -1.0f) : 0.0f;
-    kv = cf * kv;
-    fb = fma3(0.5f * Kp, kv, fb); fc = fma3(0.5f * Kq, kv, fc); fa = fma3(Ko, kv, fa);
-  }
-  {
-    const float Kp = tr.f[13], Kq = tr.f[14], Ko = tr.f[15], rp = tr.f[16];
-    const float Kf = -(Kp + Kq + Ko);
-    F3 kv = fma3(-Kq, eac, fma3(-Ko, ebc, Kf * (zf2 - zc)));  // za - zc = -eac, zb - zc = -ebc
-    const float nk2 = dot(kv, kv);
-    const float cf = nk2 > 1e-30f ? fmaf(rp, frsqrt(nk2), -1.0f) : 0.0f;
-    kv = cf * kv;
-    fc = fma3(0.5f * Kp, kv, fc); fa = fma3(0.5f * Kq, kv, fa); fb = fma3(Ko, kv, fb);
-  }
-  st3(out9, fa); st3(out9 + 3, fb); st3(out9 + 6, fc);
+  f1 = fma3(i00, Q0, i01 * Q1);
+  f2 = i11 * Q1;
 }
 
-__device__ __forceinline__ uint32_t to_tf32(float x) {
-  uint32_t r;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-  return r;
+// Bending hinge on the edge (p,q) with own opposite vertex o and the vertex f across:
+// kv = sum K_i z_i written with edges from p (rows of K sum to 0), scaled so that adding
+// K_i * kv to vertex i applies the residual  w_h K_i (r_h k/|k| - k)  (bending).
+__device__ __forceinline__ F3 hinge_vec(float Kq, float Ko, float Kf, float rp, F3 epq, F3 epo, F3 epf) {
+  const F3 kv = fma3(Kq, epq, fma3(Ko, epo, Kf * epf));
+  const float nk2 = fmaxf(dot(kv, kv), 1e-30f);
+  const float cf = fmaf(rp, frsqrt(nk2), -1.0f);
+  return cf * kv;
 }
+
 __device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], const uint32_t (&b)[2]) {
   asm volatile(
       "mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
@@ -185,258 +157,392 @@ __device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], 
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
 }
 
+// Register-resident constants of one element (npfem_internal.h: ElemConst).
+struct ElemReg {
+  uint32_t ab, cd, f12, f34;   // packed byte offsets (16 * internal id) into a cell's z4
+  float f[kElemFloats];
+};
+
+// Local step of one element for one cell: membrane residuals of its two triangles and the five
+// hinges it sees, summed per own vertex (a,b,c,d) into out4[0..3].  zc = the cell's z4 array.
+__device__ __forceinline__ void element_residual(const ElemReg& er, const unsigned char* __restrict__ zc,
+                                                 const DevParams& P, float4* __restrict__ out4) {
+  const F3 za = lds3(zc, er.ab & 0xffffu), zb = lds3(zc, er.ab >> 16);
+  const F3 zc3 = lds3(zc, er.cd & 0xffffu), zd = lds3(zc, er.cd >> 16);
+  const F3 eab = zb - za, eac = zc3 - za, ebc = zc3 - zb, ead = zd - za, ebd = zd - zb;
+  const F3 eba = {-eab.x, -eab.y, -eab.z};
+
+  // ---- membranes: t1 = (a,b,c) from a; t2 = (b,a,d) from b
+  F3 t1b, t1c, t2a, t2d;
+  membrane(eab, eac, er.f[0], er.f[1], er.f[2], er.f[3], er.f[4], P, t1b, t1c);
+  membrane(eba, ebd, er.f[5], er.f[6], er.f[7], er.f[8], er.f[9], P, t2a, t2d);
+  F3 fa = t2a - (t1b + t1c);
+  F3 fb = t1b - (t2a + t2d);
+  F3 fc = t1c;
+  F3 fd = t2d;
+
+  // ---- shared hinge (a,b | c ; d): once in full for a diamond, the element's half for a single
+  {
+    const float Kp = er.f[10], Kq = er.f[11], Ko = er.f[12];
+    const float Kf = -(Kp + Kq + Ko), he = er.f[30], hf = fmaf(2.0f, he, -1.0f);
+    const F3 kv = hinge_vec(Kq, Ko, Kf, er.f[13], eab, eac, ead);
+    fa = fma3(he * Kp, kv, fa); fb = fma3(he * Kq, kv, fb);
+    fc = fma3(Ko, kv, fc);      fd = fma3(hf * Kf, kv, fd);
+  }
+  // ---- outer hinges: half of the end-point terms, all of the own opposite vertex's term
+  {   // (b,c | a ; f1)
+    const float Kp = er.f[14], Kq = er.f[15], Ko = er.f[16];
+    const F3 zf = lds3(zc, er.f12 & 0xffffu);
+    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[17], ebc, eba, zf - zb);
+    fb = fma3(0.5f * Kp, kv, fb); fc = fma3(0.5f * Kq, kv, fc); fa = fma3(Ko, kv, fa);
+  }
+  {   // (c,a | b ; f2)
+    const float Kp = er.f[18], Kq = er.f[19], Ko = er.f[20];
+    const F3 zf = lds3(zc, er.f12 >> 16);
+    const F3 eca = {-eac.x, -eac.y, -eac.z}, ecb = {-ebc.x, -ebc.y, -ebc.z};
+    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[21], eca, ecb, zf - zc3);
+    fc = fma3(0.5f * Kp, kv, fc); fa = fma3(0.5f * Kq, kv, fa); fb = fma3(Ko, kv, fb);
+  }
+  {   // (a,d | b ; f3)
+    const float Kp = er.f[22], Kq = er.f[23], Ko = er.f[24];
+    const F3 zf = lds3(zc, er.f34 & 0xffffu);
+    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[25], ead, eab, zf - za);
+    fa = fma3(0.5f * Kp, kv, fa); fd = fma3(0.5f * Kq, kv, fd); fb = fma3(Ko, kv, fb);
+  }
+  {   // (d,b | a ; f4)
+    const float Kp = er.f[26], Kq = er.f[27], Ko = er.f[28];
+    const F3 zf = lds3(zc, er.f34 >> 16);
+    const F3 edb = {-ebd.x, -ebd.y, -ebd.z}, eda = {-ead.x, -ead.y, -ead.z};
+    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[29], edb, eda, zf - zd);
+    fd = fma3(0.5f * Kp, kv, fd); fb = fma3(0.5f * Kq, kv, fb); fa = fma3(Ko, kv, fa);
+  }
+  out4[0] = make_float4(fa.x, fa.y, fa.z, 0.0f);
+  out4[1] = make_float4(fb.x, fb.y, fb.z, 0.0f);
+  out4[2] = make_float4(fc.x, fc.y, fc.z, 0.0f);
+  out4[3] = make_float4(fd.x, fd.y, fd.z, 0.0f);
+}
+
+// grad V at a vertex = 1/6 sum over its fan of (r_i - z) x (r_i+1 - z); the first kRegList ring
+// offsets come from registers, longer fans continue from the global list.
+__device__ __forceinline__ F3 ring_gradient(const unsigned char* zc, F3 zv, int rcnt,
+                                            const uint32_t (&roff)[kRegList / 2],
+                                            const uint16_t* __restrict__ ring_tail) {
+  const F3 e0 = lds3(zc, roff[0] & 0xffffu) - zv;
+  F3 ep = e0, g = {0.f, 0.f, 0.f};
+#pragma unroll
+  for (int i = 1; i < kRegList; ++i) {
+    if (i < rcnt) {
+      const F3 e = lds3(zc, (i & 1) ? (roff[i >> 1] >> 16) : (roff[i >> 1] & 0xffffu)) - zv;
+      g = cross_acc(ep, e, g);
+      ep = e;
+    }
+  }
+  for (int i = kRegList; i < rcnt; ++i) {
+    const F3 e = lds3(zc, ring_tail[i]) - zv;
+    g = cross_acc(ep, e, g);
+    ep = e;
+  }
+  g = cross_acc(ep, e0, g);
+  return (1.0f / 6.0f) * g;
+}
 
 // ------------------------------------------------------------------------------------------
-// The fused step kernel.  MODE 1: global step with fp32 FMAs; MODE 2: 3xTF32 mma.sync.
+// The fused step kernel.  MODE 1: global step with fp32 FMAs (comparison path); MODE 2: 3xTF32
+// mma.sync on the block-sparse inverse.
 // ------------------------------------------------------------------------------------------
 template <int MODE, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  float* const z = reinterpret_cast<float*>(smem_raw + P.L.z);      // [k][n][3] current iterate (local coords)
-  float* const s = reinterpret_cast<float*>(smem_raw + P.L.s);      // [k][n][3] inertial prediction
-  float* const d = reinterpret_cast<float*>(smem_raw + P.L.d);      // [k][n][3] correction d^k
-  float* const r = reinterpret_cast<float*>(smem_raw + P.L.r);      // [2][nvb*8][8] right-hand sides
-  float* const out = reinterpret_cast<float*>(smem_raw + P.L.out);  // [T][9] triangle results / scratch
-  float* const red = reinterpret_cast<float*>(smem_raw + P.L.red);  // [5][32][4] reduction partials
-  __shared__ float vstar_s[kMaxCellsPerCta];
-  __shared__ int vactive_s[kMaxCellsPerCta];
+  unsigned char* const z4b = smem_raw + P.L.z4;                       // [k][NP] float4 iterate z
+  float* const s = reinterpret_cast<float*>(smem_raw + P.L.s);        // [3k][NP] inertial prediction
+  float* const d = reinterpret_cast<float*>(smem_raw + P.L.d);        // [3k][NP] correction d^k
+  float* const ra = reinterpret_cast<float*>(smem_raw + P.L.ra);      // rhs, A-fragment order (fp32 / hi)
+  unsigned char* const rbb = smem_raw + P.L.rb;                       // element results / rhs lo parts
+  float* const rb = reinterpret_cast<float*>(rbb);
+  float4* const red = reinterpret_cast<float4*>(smem_raw + P.L.red);  // [k][32] partial sums
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
-  const int n = P.n, T = P.T, nvb = P.nvb;
+  const int n = P.n, E = P.E, nvb = P.nvb, NP = nvb * 8;
   const int cell0 = blockIdx.x * P.k;
   const int kact = min(P.k, P.n_cells - cell0);
-  const int n3 = 3 * n;
+  const int cellz = NP * 16;                      // bytes of one cell's z4
 
-  // ---- per-thread constants: up to two triangles and one vertex
-  TriReg tr[kTrisPerThread];
+  // ---- per-thread constants: one element and one vertex
+  const bool is_e = tid < E, isv = tid < n, isvp = tid < NP;
+  ElemReg er;
+  {
+    const int e = is_e ? tid : 0;
+    er.ab = P.elem_ids[e]; er.cd = P.elem_ids[E + e];
+    er.f12 = P.elem_ids[2 * E + e]; er.f34 = P.elem_ids[3 * E + e];
 #pragma unroll
-  for (int j = 0; j < kTrisPerThread; ++j) {
-    const int t = tid + j * blockDim.x;
-    if (t < T) {
-      tr[j].ab = P.tri_ids[t] | (uint32_t(P.tri_ids[T + t]) << 16);
-      tr[j].cf0 = P.tri_ids[2 * T + t] | (uint32_t(P.tri_ids[3 * T + t]) << 16);
-      tr[j].f12 = P.tri_ids[4 * T + t] | (uint32_t(P.tri_ids[5 * T + t]) << 16);
-#pragma unroll
-      for (int q = 0; q < kTriFloats; ++q) tr[j].f[q] = P.tri_f[q * T + t];
-    } else {
-      tr[j].ab = tr[j].cf0 = tr[j].f12 = 0;
-#pragma unroll
-      for (int q = 0; q < kTriFloats; ++q) tr[j].f[q] = 0.0f;
-    }
+    for (int q = 0; q < kElemFloats; ++q) er.f[q] = P.elem_f[q * E + e];
   }
-  const bool isv = tid < n;
-  const int v = isv ? tid : 0;
+  const int v = isvp ? tid : 0;
   const int vext = P.perm[v];
   const float h2m = P.h2_over_m[v], mh2 = P.m_over_h2[v];
-  const int inc0 = P.inc_ptr[v], inc1 = P.inc_ptr[v + 1];
   const float h = P.h;
+  int icnt = 0, rcnt = 0;
+  uint32_t ioff[kRegList / 2] = {0, 0, 0}, roff[kRegList / 2] = {0, 0, 0};
+  const uint16_t* inc_tail = P.inc_off;
+  const uint16_t* ring_tail = P.ring_off;
+  if (isv) {
+    const int i0 = P.inc_ptr[v], r0 = P.ring_ptr[v];
+    icnt = P.inc_ptr[v + 1] - i0;
+    rcnt = P.ring_ptr[v + 1] - r0;
+    inc_tail += i0;
+    ring_tail += r0;
+#pragma unroll
+    for (int i = 0; i < kRegList; ++i) {
+      const uint32_t io = i < icnt ? inc_tail[i] : 0u, ro = i < rcnt ? ring_tail[i] : 0u;
+      ioff[i >> 1] |= io << (16 * (i & 1));
+      roff[i >> 1] |= ro << (16 * (i & 1));
+    }
+  }
+  // float index of (vertex v, rhs column 0) in the A-fragment layout:
+  //   block jb = v/8 holds 32 lanes x float4; lane = (m&7)*4 + (v&3), component = 2*((v&7)>>2) + (m>>3)
+  const int fbase = ((v >> 3) * 32 + (v & 3)) * 4 + 2 * ((v & 7) >> 2);
 
-  // zero the right-hand-side buffer once: padding vertices, the 16th column and the columns of
-  // missing cells are never written afterwards
-  for (int i = tid; i < 2 * nvb * 64; i += blockDim.x) r[i] = 0.0f;
+  // ---- zero the state that padding vertices / missing cells never write
+  for (int i = tid; i < NP * 16; i += blockDim.x) ra[i] = 0.0f;
+  for (int i = tid; i < 3 * P.k * NP; i += blockDim.x) { s[i] = 0.0f; d[i] = 0.0f; }
+  for (int i = tid; i < P.k * NP; i += blockDim.x)
+    reinterpret_cast<float4*>(z4b)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
   // ---- prologue: load state, centroid, local coordinates, inertial prediction
-  for (int c = 0; c < kact; ++c) {
-    float sx = 0.f, sy = 0.f, sz = 0.f;
-    if (isv) {
-      const float* px = P.pos + (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
-      sx = px[0]; sy = px[1]; sz = px[2];
+  {
+    float* const scr = rb;   // [k][32][4] scratch
+    for (int c = 0; c < kact; ++c) {
+      float sx = 0.f, sy = 0.f, sz = 0.f;
+      if (isv) {
+        const float* px = P.pos + (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
+        sx = px[0]; sy = px[1]; sz = px[2];
+      }
+      sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
+      if (lane == 0) { float* q = scr + (c * 32 + warp) * 4; q[0] = sx; q[1] = sy; q[2] = sz; }
     }
-    sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
-    if (lane == 0) { float* q = red + (c * 32 + warp) * 4; q[0] = sx; q[1] = sy; q[2] = sz; }
-  }
-  __syncthreads();
-  for (int c = 0; c < kact; ++c) {
-    const float* q = red + (c * 32 + lane) * 4;
-    float cx = lane < nwarps ? q[0] : 0.f, cy = lane < nwarps ? q[1] : 0.f, cz = lane < nwarps ? q[2] : 0.f;
-    cx = warp_sum(cx); cy = warp_sum(cy); cz = warp_sum(cz);
-    const float invn = 1.0f / (float)n;
-    cx *= invn; cy *= invn; cz *= invn;
-    if (isv) {
-      const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
-      const F3 x = ld3(P.pos + g), vv = ld3(P.vel + g), ff = ld3(P.fext + g);
-      const F3 u0 = {fmaf(h, vv.x, h2m * ff.x), fmaf(h, vv.y, h2m * ff.y), fmaf(h, vv.z, h2m * ff.z)};
-      const F3 y = {x.x - cx, x.y - cy, x.z - cz};
-      const F3 sv = y + u0;
-      const int o = c * n3 + 3 * v;
-      st3(s + o, sv); st3(z + o, sv);
-      d[o] = 0.f; d[o + 1] = 0.f; d[o + 2] = 0.f;
+    __syncthreads();
+    for (int c = 0; c < kact; ++c) {
+      const float* q = scr + (c * 32 + lane) * 4;
+      float cx = lane < nwarps ? q[0] : 0.f, cy = lane < nwarps ? q[1] : 0.f, cz = lane < nwarps ? q[2] : 0.f;
+      cx = warp_sum(cx); cy = warp_sum(cy); cz = warp_sum(cz);
+      const float invn = 1.0f / (float)n;
+      cx *= invn; cy *= invn; cz *= invn;
+      if (isv) {
+        const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
+        const float x0 = P.pos[g], x1 = P.pos[g + 1], x2 = P.pos[g + 2];
+        const float sx = (x0 - cx) + fmaf(h, P.vel[g], h2m * P.fext[g]);
+        const float sy = (x1 - cy) + fmaf(h, P.vel[g + 1], h2m * P.fext[g + 1]);
+        const float sz = (x2 - cz) + fmaf(h, P.vel[g + 2], h2m * P.fext[g + 2]);
+        s[(3 * c) * NP + v] = sx; s[(3 * c + 1) * NP + v] = sy; s[(3 * c + 2) * NP + v] = sz;
+        reinterpret_cast<float4*>(z4b)[c * NP + v] = make_float4(sx, sy, sz, 0.f);
+      }
     }
+    __syncthreads();
   }
-  __syncthreads();
 
   // ---- iterations
+  const float vol_tol = kVolTol * P.V0;
+  const float vol_dlen = kVolDTol * cbrtf(P.V0);
+  const float vol_dtol2 = (float)n * vol_dlen * vol_dlen;
+  const bool use_vol = P.w_volume > 0.0f;
   for (int it = 0; it < P.n_iters; ++it) {
-    // local step, elastic part: triangles -> out, vertices gather -> r = e - (m/h^2) d
+    // local step.  Pipeline over the CTA's cells, two barriers per cell:
+    //   [elements(c) -> out] | [vertices(c): gather out, grad V, partial sums] | [elements(c+1);
+    //   finish(c): volume multiplier, right-hand side] | ...
+    if (is_e) element_residual(er, z4b, P, reinterpret_cast<float4*>(rbb) + 4 * tid);
+    __syncthreads();
     for (int c = 0; c < kact; ++c) {
-      const float* zc = z + c * n3;
-#pragma unroll
-      for (int j = 0; j < kTrisPerThread; ++j) {
-        const int t = tid + j * blockDim.x;
-        if (t < T) triangle_residual(tr[j], zc, P, out + 9 * t);
-      }
-      __syncthreads();
+      const unsigned char* zc = z4b + c * cellz;
+      F3 ev = {0.f, 0.f, 0.f}, g = {0.f, 0.f, 0.f}, zv = {0.f, 0.f, 0.f};
+      float S1 = 0.f, S2 = 0.f;
       if (isv) {
-        float ex = 0.f, ey = 0.f, ez = 0.f;
-        for (int i = inc0; i < inc1; ++i) {
-          const float* o = out + P.inc_out[i];
-          ex += o[0]; ey += o[1]; ez += o[2];
+#pragma unroll
+        for (int i = 0; i < kRegList; ++i) {
+          if (i < icnt) {
+            const F3 o = lds3(rbb, (i & 1) ? (ioff[i >> 1] >> 16) : (ioff[i >> 1] & 0xffffu));
+            ev = ev + o;
+          }
         }
-        const int o = c * n3 + 3 * v;
-        const int m = 3 * c;
-        float* rr = r + (size_t)v * 8;
-        const int half = nvb * 64;
-        rr[((m) >> 3) * half + ((m) & 7)] = fmaf(-mh2, d[o], ex);
-        rr[((m + 1) >> 3) * half + ((m + 1) & 7)] = fmaf(-mh2, d[o + 1], ey);
-        rr[((m + 2) >> 3) * half + ((m + 2) & 7)] = fmaf(-mh2, d[o + 2], ez);
+        for (int i = kRegList; i < icnt; ++i) ev = ev + lds3(rbb, inc_tail[i]);
+        if (use_vol) {
+          zv = lds3(zc, v * 16);
+          g = ring_gradient(zc, zv, rcnt, roff, ring_tail);
+          S1 = dot(zv, g);
+          S2 = dot(g, g);
+        }
       }
-      __syncthreads();
-    }
+      if (use_vol) {
+        S1 = warp_sum(S1); S2 = warp_sum(S2);
+        if (lane == 0) red[c * 32 + warp] = make_float4(S1, S2, 0.f, 0.f);
+      }
+      __syncthreads();   // out consumed, partial sums complete
 
-    // local step, volume part: D = lambda * grad V(z + D), vol_iters fixed-point sweeps
-    // (D <- ((g.D - C)/(g.g)) g; grad V at a vertex = 1/6 sum of ring cross products,
-    //  V = 1/3 sum_v x_v . g_v for the closed surface).  out[] is free now and holds D / g.
-    if (P.w_volume > 0.0f) {
-      float* const scr = out;   // [k][n][3]
-      for (int vi = 0; vi < P.vol_iters; ++vi) {
-        for (int c = 0; c < kact; ++c) {
-          float S1 = 0.f, S2 = 0.f, S3 = 0.f;
-          if (isv && (vi == 0 || vactive_s[c])) {
-            const float* zc = z + c * n3;
-            const int o = c * n3 + 3 * v;
-            const F3 zv = ld3(zc + 3 * v);
-            F3 g = {0.f, 0.f, 0.f};
-            F3 eprev = ld3(zc + 3 * P.inc_ring[inc1 - 1]) - zv;
-            for (int i = inc0; i < inc1; ++i) {
-              const F3 e = ld3(zc + 3 * P.inc_ring[i]) - zv;
-              const F3 cr = cross(eprev, e);
-              g = g + cr;
-              eprev = e;
-            }
-            g = (1.0f / 6.0f) * g;
-            S1 = dot(zv, g);
-            S2 = dot(g, g);
-            if (vi > 0) S3 = dot(g, ld3(scr + o));
-            st3(scr + o, g);
-          }
-          S1 = warp_sum(S1); S2 = warp_sum(S2); S3 = warp_sum(S3);
-          if (lane == 0) { float* q = red + (c * 32 + warp) * 4; q[0] = S1; q[1] = S2; q[2] = S3; }
-        }
-        __syncthreads();
-        for (int c = 0; c < kact; ++c) {
-          const float* q = red + (c * 32 + lane) * 4;
-          float S1 = lane < nwarps ? q[0] : 0.f, S2 = lane < nwarps ? q[1] : 0.f, S3 = lane < nwarps ? q[2] : 0.f;
-          S1 = warp_sum(S1); S2 = warp_sum(S2); S3 = warp_sum(S3);
-          const float V = S1 * (1.0f / 3.0f);
-          float vstar;
-          bool active;
-          if (vi == 0) {
-            vstar = fminf(fmaxf(V, P.Vmin), P.Vmax);
-            active = (V != vstar);
-          } else {
-            vstar = vstar_s[c];
-            active = vactive_s[c] != 0;
-          }
-          const float lambda = (active && S2 > 0.f) ? (S3 - (V - vstar)) / S2 : 0.f;
+      if (c + 1 < kact && is_e)
+        element_residual(er, z4b + (c + 1) * cellz, P, reinterpret_cast<float4*>(rbb) + 4 * tid);
+
+      // finish(c): D = lambda grad V(z + D), iterated (D <- ((g.D - C)/(g.g)) g,
+      // V = 1/3 sum_v z_v . g_v for the closed surface); stops early by kVolTol
+      F3 D = {0.f, 0.f, 0.f};
+      if (use_vol) {
+        float4 p4 = lane < nwarps ? red[c * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+        S1 = warp_sum(p4.x); S2 = warp_sum(p4.y);
+        const float V = S1 * (1.0f / 3.0f);
+        const float vstar = fminf(fmaxf(V, P.Vmin), P.Vmax);
+        float C = V - vstar;
+        const bool active = (V != vstar);
+        float lambda = (active && S2 > 0.f) ? -C / S2 : 0.f;
+        D = lambda * g;
+        bool moved = false;
+        // Another pass only while it can still matter: after the first, first-order correction the
+        // remaining error is second order in the violation (kVolTol); later, when the last pass
+        // moved D by less than vol_dtol (rms per vertex).  |D_j+1 - D_j|^2 follows from the sums
+        // already reduced: |D_j+1|^2 + |D_j|^2 - 2 lambda_j+1 (g_j+1 . D_j).
+        bool more = fabsf(C) > vol_tol;
+        float D2prev = lambda * lambda * S2;
+        for (int pass = 1; pass < P.vol_iters && active && more; ++pass) {
+          // CTA-uniform branch: every warp reduced the same partial sums in the same order
+          float4* z4c = reinterpret_cast<float4*>(z4b + c * cellz);
+          const F3 zz = zv + D;
+          if (isv) z4c[v] = make_float4(zz.x, zz.y, zz.z, 0.f);
+          moved = true;
+          __syncthreads();
+          float S3 = 0.f;
+          S1 = 0.f; S2 = 0.f;
           if (isv) {
-            const int o = c * n3 + 3 * v;
-            const F3 D = lambda * ld3(scr + o);
-            st3(scr + o, D);
-            if (vi + 1 < P.vol_iters && active) {
-              const F3 zz = (ld3(s + o) + ld3(d + o)) + D;
-              st3(z + o, zz);
-            }
+            g = ring_gradient(zc, zz, rcnt, roff, ring_tail);
+            S1 = dot(zz, g); S2 = dot(g, g); S3 = dot(g, D);
           }
-          if (vi == 0 && tid == 0) { vstar_s[c] = vstar; vactive_s[c] = active ? 1 : 0; }
+          S1 = warp_sum(S1); S2 = warp_sum(S2); S3 = warp_sum(S3);
+          if (lane == 0) red[c * 32 + warp] = make_float4(S1, S2, S3, 0.f);
+          __syncthreads();
+          p4 = lane < nwarps ? red[c * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+          S1 = warp_sum(p4.x); S2 = warp_sum(p4.y); S3 = warp_sum(p4.z);
+          C = S1 * (1.0f / 3.0f) - vstar;
+          lambda = S2 > 0.f ? (S3 - C) / S2 : 0.f;
+          D = lambda * g;
+          const float D2new = lambda * lambda * S2;
+          more = (D2new + D2prev - 2.0f * lambda * S3) > vol_dtol2;
+          D2prev = D2new;
+          __syncthreads();   // red[c] is rewritten by the next pass
         }
-        __syncthreads();
+        if (moved && isv) reinterpret_cast<float4*>(z4b + c * cellz)[v] = make_float4(zv.x, zv.y, zv.z, 0.f);
       }
       if (isv) {
-        const int half = nvb * 64;
-        float* rr = r + (size_t)v * 8;
-        for (int c = 0; c < kact; ++c) {
-          const int o = c * n3 + 3 * v;
-          const int m = 3 * c;
-          // residual of the volume term: w_vol (P_v - z) = w_vol D
-          rr[((m) >> 3) * half + ((m) & 7)] += P.w_volume * scr[o];
-          rr[((m + 1) >> 3) * half + ((m + 1) & 7)] += P.w_volume * scr[o + 1];
-          rr[((m + 2) >> 3) * half + ((m + 2) & 7)] += P.w_volume * scr[o + 2];
-        }
+        // right-hand side of the global step, r = e - (m/h^2) d with e including w_vol D
+        const int m = 3 * c;
+        const float r0 = fmaf(P.w_volume, D.x, fmaf(-mh2, d[m * NP + v], ev.x));
+        const float r1 = fmaf(P.w_volume, D.y, fmaf(-mh2, d[(m + 1) * NP + v], ev.y));
+        const float r2 = fmaf(P.w_volume, D.z, fmaf(-mh2, d[(m + 2) * NP + v], ev.z));
+        ra[fbase + ((m) & 7) * 16 + ((m) >> 3)] = r0;
+        ra[fbase + ((m + 1) & 7) * 16 + ((m + 1) >> 3)] = r1;
+        ra[fbase + ((m + 2) & 7) * 16 + ((m + 2) >> 3)] = r2;
       }
-      __syncthreads();
+      __syncthreads();   // out(c+1) complete; z4 of cell c restored
     }
 
-    // global step: d += T r, with T in 8x8 blocks; one warp per block of 8 output vertices
-    const int mlim = 3 * kact;
-    if (MODE == 1) {
-      const int g = lane >> 2, q4 = lane & 3;
-      const float* rbase0 = r + (q4 >> 1) * nvb * 64 + (q4 & 1) * 4;
-      for (int ib = warp; ib < nvb; ib += nwarps) {
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-        const int b1 = P.blk_ptr[ib + 1];
-        for (int b = P.blk_ptr[ib]; b < b1; ++b) {
-          const int jb = P.blk_col[b];
-          const float4* tv = reinterpret_cast<const float4*>(P.blk_val + (size_t)b * 64 + g * 8);
-          const float4 t0 = __ldg(tv), t1 = __ldg(tv + 1);
-          const float tk[8] = {t0.x, t0.z, t1.x, t1.z, t0.y, t0.w, t1.y, t1.w};   // k = 0..7
-          const float* rb = rbase0 + jb * 64;
+    // split the right-hand sides into tf32 high and low parts (hi in place, lo over the dead
+    // element buffer).  Round-to-nearest on the 13 dropped mantissa bits; lo = x - hi is exact.
+    if (isvp) {
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk) {
-            const float4 r4 = *reinterpret_cast<const float4*>(rb + kk * 8);
-            a0 = fmaf(tk[kk], r4.x, a0); a1 = fmaf(tk[kk], r4.y, a1);
-            a2 = fmaf(tk[kk], r4.z, a2); a3 = fmaf(tk[kk], r4.w, a3);
-          }
-        }
-        const int i = ib * 8 + g;
-        const float acc[4] = {a0, a1, a2, a3};
-        if (i < n) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int m = 4 * q4 + e;
-            if (m < mlim) {
-              const int c = m / 3, comp = m - 3 * c;
-              const int o = c * n3 + 3 * i + comp;
-              const float dn = d[o] + acc[e];
-              d[o] = dn;
-              z[o] = s[o] + dn;
-            }
-          }
-        }
+      for (int m = 0; m < kRhs; ++m) {
+        const int idx = fbase + (m & 7) * 16 + (m >> 3);
+        const float x = ra[idx];
+        const float hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+        ra[idx] = hi;
+        rb[idx] = x - hi;
       }
-    } else {
-      const int g = lane >> 2, t4 = lane & 3;
-      const int half = nvb * 64;
+    }
+    __syncthreads();
+
+    // global step: d += T r with T = A_sys^-1 in 8x8 blocks.  One warp per block of 8 output
+    // vertices: mma m16n8k8, M = the 16 right-hand-side columns, N = 8 output vertices, K = 8 source
+    // vertices per operator block; A fragments (hi, lo) are one LDS.128 each, the operator block
+    // comes straight from L2 and is split in registers (the tensor core ignores the low 13 bits).
+    {
+      const int g8 = lane >> 2, t4 = lane & 3;
+      const float4* const Ahi = reinterpret_cast<const float4*>(ra) + lane;
+      const float4* const Alo = reinterpret_cast<const float4*>(rb) + lane;
+      float* const z4f = reinterpret_cast<float*>(z4b);
+      // rows of the accumulator this lane owns: m = g8 and g8 + 8 (row 15 is the padding column)
+      const int m0 = g8, m1 = g8 + 8;
+      const int zo0 = ((m0 / 3) * NP) * 4 + (m0 % 3), zo1 = ((m1 / 3) * NP) * 4 + (m1 % 3);
       for (int ib = warp; ib < nvb; ib += nwarps) {
         float acc[4] = {0.f, 0.f, 0.f, 0.f};
-        const int b1 = P.blk_ptr[ib + 1];
-        for (int b = P.blk_ptr[ib]; b < b1; ++b) {
-          const int jb = P.blk_col[b];
-          const float2 tb = __ldg(reinterpret_cast<const float2*>(P.blk_val + (size_t)b * 64) + lane);
-          const float* rb = r + jb * 64 + t4 * 8 + g;
-          const float av[4] = {rb[0], rb[half], rb[32], rb[half + 32]};
-          uint32_t ahi[4], alo[4], bhi[2], blo[2];
+        const int b0 = P.blk_ptr[ib], b1 = P.blk_ptr[ib + 1];
+        if (MODE == 2) {
+          const float2* tv = reinterpret_cast<const float2*>(P.blk_val) + (size_t)b0 * 32 + lane;
+          for (int bb = b0; bb < b1; bb += 32) {
+            const int nb = min(32, b1 - bb);          // multiple of 4 (rows are padded)
+            const int colv = lane < nb ? (int)P.blk_col[bb + lane] * 32 : 0;
+            float2 cur[4], nxt[4];
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            ahi[e] = to_tf32(av[e]);
-            alo[e] = to_tf32(av[e] - __uint_as_float(ahi[e]));
+            for (int u = 0; u < 4; ++u) cur[u] = __ldg(tv + u * 32);
+            for (int j = 0; j < nb; j += 4) {
+              tv += 128;
+              if (j + 4 < nb) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) nxt[u] = __ldg(tv + u * 32);
+              }
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const int col = __shfl_sync(0xffffffffu, colv, j + u);
+                const float4 ah = Ahi[col], al = Alo[col];
+                const uint32_t ahi[4] = {__float_as_uint(ah.x), __float_as_uint(ah.y),
+                                         __float_as_uint(ah.z), __float_as_uint(ah.w)};
+                const uint32_t alo[4] = {__float_as_uint(al.x), __float_as_uint(al.y),
+                                         __float_as_uint(al.z), __float_as_uint(al.w)};
+                const uint32_t bx = __float_as_uint(cur[u].x) & 0xffffe000u;
+                const uint32_t by = __float_as_uint(cur[u].y) & 0xffffe000u;
+                const uint32_t bhi[2] = {bx, by};
+                const uint32_t blo[2] = {__float_as_uint(cur[u].x - __uint_as_float(bx)),
+                                         __float_as_uint(cur[u].y - __uint_as_float(by))};
+                mma_tf32(acc, alo, bhi);
+                mma_tf32(acc, ahi, blo);
+                mma_tf32(acc, ahi, bhi);
+              }
+#pragma unroll
+              for (int u = 0; u < 4; ++u) cur[u] = nxt[u];
+            }
           }
-          bhi[0] = to_tf32(tb.x); blo[0] = to_tf32(tb.x - __uint_as_float(bhi[0]));
-          bhi[1] = to_tf32(tb.y); blo[1] = to_tf32(tb.y - __uint_as_float(bhi[1]));
-          mma_tf32(acc, alo, bhi);
-          mma_tf32(acc, ahi, blo);
-          mma_tf32(acc, ahi, bhi);
+        } else {
+          // fp32 comparison path: the same sums with plain FMAs, operands re-read per term
+          for (int b = b0; b < b1; ++b) {
+            const int col = (int)P.blk_col[b] * 32;
+            const float* hi = ra + col * 4;
+            const float* lo = rb + col * 4;
+            const float* tb = P.blk_val + (size_t)b * 64;
+#pragma unroll
+            for (int kk = 0; kk < 8; ++kk) {
+              // A(m, kk) sits in lane (m&7)*4 + (kk&3), component 2*(kk>>2) + (m>>3)
+              const int ia = (g8 * 4 + (kk & 3)) * 4 + 2 * (kk >> 2);
+              const float a0 = hi[ia] + lo[ia], a1 = hi[ia + 1] + lo[ia + 1];
+              // B(kk, i) sits at 2*((i<<2) | (kk&3)) + (kk>>2)
+              const float bq0 = __ldg(tb + 2 * (((2 * t4) << 2) | (kk & 3)) + (kk >> 2));
+              const float bq1 = __ldg(tb + 2 * (((2 * t4 + 1) << 2) | (kk & 3)) + (kk >> 2));
+              acc[0] = fmaf(a0, bq0, acc[0]); acc[1] = fmaf(a0, bq1, acc[1]);
+              acc[2] = fmaf(a1, bq0, acc[2]); acc[3] = fmaf(a1, bq1, acc[3]);
+            }
+          }
         }
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const int m = g + ((e & 2) ? 8 : 0);
-          const int i = ib * 8 + 2 * t4 + (e & 1);
-          if (m < mlim && i < n) {
-            const int c = m / 3, comp = m - 3 * c;
-            const int o = c * n3 + 3 * i + comp;
-            const float dn = d[o] + acc[e];
-            d[o] = dn;
-            z[o] = s[o] + dn;
-          }
+        // epilogue: d += acc, z = s + d for the lane's two rows and two adjacent output vertices
+        const int i0 = ib * 8 + 2 * t4;
+        if (m0 < 3 * P.k) {
+          float2* dp = reinterpret_cast<float2*>(d + m0 * NP + i0);
+          const float2 sv = *reinterpret_cast<const float2*>(s + m0 * NP + i0);
+          float2 dv = *dp;
+          dv.x += acc[0]; dv.y += acc[1];
+          *dp = dv;
+          z4f[zo0 + i0 * 4] = sv.x + dv.x;
+          z4f[zo0 + i0 * 4 + 4] = sv.y + dv.y;
+        }
+        if (m1 < 3 * P.k) {
+          float2* dp = reinterpret_cast<float2*>(d + m1 * NP + i0);
+          const float2 sv = *reinterpret_cast<const float2*>(s + m1 * NP + i0);
+          float2 dv = *dp;
+          dv.x += acc[2]; dv.y += acc[3];
+          *dp = dv;
+          z4f[zo1 + i0 * 4] = sv.x + dv.x;
+          z4f[zo1 + i0 * 4 + 4] = sv.y + dv.y;
         }
       }
     }
@@ -445,15 +551,15 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
 
   // ---- epilogue: x_n+1 = x_n + (u0 + d), v_n+1 = (u0 + d)/h
   if (isv) {
+    const float invh = 1.0f / h;
     for (int c = 0; c < kact; ++c) {
       const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
-      const F3 x = ld3(P.pos + g), vv = ld3(P.vel + g), ff = ld3(P.fext + g);
-      const int o = c * n3 + 3 * v;
-      const F3 inc = {fmaf(h, vv.x, h2m * ff.x) + d[o], fmaf(h, vv.y, h2m * ff.y) + d[o + 1],
-                      fmaf(h, vv.z, h2m * ff.z) + d[o + 2]};
-      st3(P.pos + g, x + inc);
-      const F3 vn = {inc.x / h, inc.y / h, inc.z / h};
-      st3(P.vel + g, vn);
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        const float inc = fmaf(h, P.vel[g + q], h2m * P.fext[g + q]) + d[(3 * c + q) * NP + v];
+        P.pos[g + q] += inc;
+        P.vel[g + q] = inc * invh;
+      }
     }
   }
 }
@@ -468,7 +574,7 @@ cudaError_t configure_kernels(int smem_bytes) {
   e = cudaFuncSetAttribute(npfem_step_kernel<MODE, MAXT>,                                       \
                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);            \
   if (e != cudaSuccess) return e;
-  NPFEM_CFG(1, 704) NPFEM_CFG(1, 1024) NPFEM_CFG(2, 704) NPFEM_CFG(2, 1024)
+  NPFEM_CFG(1, 672) NPFEM_CFG(1, 1024) NPFEM_CFG(2, 672) NPFEM_CFG(2, 1024)
 #undef NPFEM_CFG
   return cudaSuccess;
 }
@@ -477,9 +583,9 @@ cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mod
                         cudaStream_t stream) {
   if (p.n_cells <= 0) return cudaSuccess;
   const int grid = (p.n_cells + p.k - 1) / p.k;
-  if (threads <= 704) {
-    if (mode == 2) npfem_step_kernel<2, 704><<<grid, threads, smem_bytes, stream>>>(p);
-    else npfem_step_kernel<1, 704><<<grid, threads, smem_bytes, stream>>>(p);
+  if (threads <= 672) {
+    if (mode == 2) npfem_step_kernel<2, 672><<<grid, threads, smem_bytes, stream>>>(p);
+    else npfem_step_kernel<1, 672><<<grid, threads, smem_bytes, stream>>>(p);
   } else {
     if (mode == 2) npfem_step_kernel<2, 1024><<<grid, threads, smem_bytes, stream>>>(p);
     else npfem_step_kernel<1, 1024><<<grid, threads, smem_bytes, stream>>>(p);

@@ -6,22 +6,31 @@
 
 namespace npfem {
 
+// The volume projection stops iterating once the violation |V - V*| it has just corrected to first
+// order is below kVolTol * V0: the step converges quadratically, so the remaining violation is
+// then below the fp32 resolution of V itself (A-17).
+constexpr float kVolTol = 2e-4f;
+// Later passes stop once the last one changed the projection by less than kVolDTol * V0^(1/3)
+// (rms per vertex): below the fp32 resolution of the cell-local coordinates.
+constexpr float kVolDTol = 5e-8f;
+
 // Everything the fused step kernel needs, passed by value.  Pointers are device pointers.
 struct DevParams {
-  int n, T, nvb, k, n_cells, cell_stride, n_iters, vol_iters;
+  int n, E, nvb, k, n_cells, cell_stride, n_iters, vol_iters;
   float h, w_volume, V0, Vmin, Vmax;       // Vmin/Vmax = v_min*V0, v_max*V0
   float s_min, s_max, a_min, a_max;
-  const uint16_t* perm;                    // [n] internal -> caller vertex
-  const uint16_t* tri_ids;                 // [6][T]  structure of arrays
-  const float* tri_f;                      // [17][T] structure of arrays
-  const float* h2_over_m;                  // [n]
-  const float* m_over_h2;                  // [n]
+  const uint16_t* perm;                    // [NP] internal -> caller vertex (padding: 0)
+  const uint32_t* elem_ids;                // [4][E] packed byte offsets 16*id: (a,b) (c,d) (f1,f2) (f3,f4)
+  const float* elem_f;                     // [kElemFloats][E] structure of arrays
+  const float* h2_over_m;                  // [NP]
+  const float* m_over_h2;                  // [NP]
   const uint16_t* inc_ptr;                 // [n+1]
-  const uint16_t* inc_out;                 // [3T]
-  const uint16_t* inc_ring;                // [3T]
+  const uint16_t* inc_off;                 // byte offsets into the element result buffer
+  const uint16_t* ring_ptr;                // [n+1]
+  const uint16_t* ring_off;                // byte offsets into one cell's z4
   const int* blk_ptr;                      // [nvb+1]
-  const uint16_t* blk_col;                 // [n_op_blocks]
-  const float* blk_val;                    // [n_op_blocks][64]
+  const uint16_t* blk_col;                 // [n_blocks_padded]
+  const float* blk_val;                    // [n_blocks_padded][64]
   float* pos;
   float* vel;
   const float* fext;

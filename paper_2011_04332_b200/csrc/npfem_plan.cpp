@@ -349,10 +349,14 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
         bmask[(size_t)(P->iperm[i] / 8) * nvb + P->iperm[j] / 8] = 1;
       }
   P->op_nnz = nnz;
+  // rows of blocks are padded with all-zero blocks to a multiple of 4 so that the kernel's
+  // unrolled, software-pipelined block loop needs no tail handling
   P->blk_ptr.assign(nvb + 1, 0);
   P->blk_col.clear();
   P->blk_val.clear();
+  P->n_op_blocks = 0;
   for (int ib = 0; ib < nvb; ++ib) {
+    int row_blocks = 0;
     for (int jb = 0; jb < nvb; ++jb) {
       if (!bmask[(size_t)ib * nvb + jb]) continue;
       P->blk_col.push_back((uint16_t)jb);
@@ -365,11 +369,18 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
           if (i < n && j < n)
             P->blk_val[base + 2 * l + r] = (float)Tinv[(size_t)P->perm[i] * n + P->perm[j]];
         }
+      ++row_blocks;
+      ++P->n_op_blocks;
+    }
+    while (row_blocks % 4) {
+      P->blk_col.push_back((uint16_t)ib);
+      P->blk_val.resize(P->blk_val.size() + 64, 0.0f);
+      ++row_blocks;
     }
     P->blk_ptr[ib + 1] = (int32_t)P->blk_col.size();
   }
 
-  // ---- per-vertex constants and cyclic incidence lists (internal numbering)
+  // ---- per-vertex constants (internal numbering)
   P->h2_over_m.resize(n);
   P->m_over_h2.resize(n);
   for (int i = 0; i < n; ++i) {
@@ -377,53 +388,206 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     P->h2_over_m[i] = (float)(dt * dt / m);
     P->m_over_h2[i] = (float)(m * ih2);
   }
-  // internal triangle order: by smallest internal vertex id, then by the sum
-  std::vector<int> torder(T);
-  std::iota(torder.begin(), torder.end(), 0);
-  auto tkey = [&](int t) {
-    int a = P->iperm[tris[3 * t]], b = P->iperm[tris[3 * t + 1]], c = P->iperm[tris[3 * t + 2]];
-    return std::make_pair(std::min(a, std::min(b, c)), a + b + c);
-  };
-  std::sort(torder.begin(), torder.end(), [&](int p, int q) {
-    auto kp = tkey(p), kq = tkey(q);
-    return kp != kq ? kp < kq : p < q;
-  });
-  std::vector<int> tint(T);   // caller triangle -> internal triangle
-  for (int ti = 0; ti < T; ++ti) tint[torder[ti]] = ti;
 
-  P->tri.assign(T, TriConst{});
-  for (int ti = 0; ti < T; ++ti) {
-    int t = torder[ti];
-    TriConst& tc = P->tri[ti];
-    int ve[3] = {tris[3 * t], tris[3 * t + 1], tris[3 * t + 2]};
-    for (int s = 0; s < 3; ++s) tc.ids[s] = (uint16_t)P->iperm[ve[s]];
-    tc.f[0] = (float)P->tri_dminv[3 * t];
-    tc.f[1] = (float)P->tri_dminv[3 * t + 1];
-    tc.f[2] = (float)P->tri_dminv[3 * t + 2];
-    tc.f[3] = (float)(mat->k_strain * P->tri_area[t]);
-    tc.f[4] = (float)(mat->k_area * P->tri_area[t]);
-    for (int e = 0; e < 3; ++e) {
-      int p = ve[e], q = ve[(e + 1) % 3], oo = ve[(e + 2) % 3];
-      int far = opposite(q, p);
-      tc.ids[3 + e] = (uint16_t)P->iperm[far];
-      int hh = hinge_of[(size_t)p * n + q];
-      const int32_t* hv = &P->hinge_verts[4 * (size_t)hh];
-      const double* K = &P->hinge_K[4 * (size_t)hh];
-      double sw = std::sqrt(P->hinge_wr[2 * (size_t)hh]);
-      auto Kof = [&](int vtx) {
-        for (int i = 0; i < 4; ++i)
-          if (hv[i] == vtx) return K[i];
-        return 0.0;
-      };
-      tc.f[5 + 4 * e + 0] = (float)(sw * Kof(p));
-      tc.f[5 + 4 * e + 1] = (float)(sw * Kof(q));
-      tc.f[5 + 4 * e + 2] = (float)(sw * Kof(oo));
-      tc.f[5 + 4 * e + 3] = (float)(sw * P->hinge_wr[2 * (size_t)hh + 1]);
+  // ---- elements: pair triangles across shared edges (a matching of the dual graph, which is
+  //      cubic and bridgeless for a closed manifold, so a perfect matching exists; greedy by
+  //      fewest free neighbours, then augmenting paths; whatever stays unmatched becomes a
+  //      single-triangle element).  Triangle neighbour across edge slot e: the triangle holding
+  //      the reversed directed edge.
+  auto tnbr = [&](int t, int e) {
+    int u = tris[3 * t + e], v = tris[3 * t + (e + 1) % 3];
+    return (int)etri[(size_t)v * n + u];
+  };
+  std::vector<int> mate(T, -1);
+  {
+    auto tkey = [&](int t) {
+      int a = P->iperm[tris[3 * t]], b = P->iperm[tris[3 * t + 1]], c = P->iperm[tris[3 * t + 2]];
+      return std::make_pair(std::min(a, std::min(b, c)), a + b + c);
+    };
+    std::vector<int> order(T);
+    std::iota(order.begin(), order.end(), 0);
+    std::sort(order.begin(), order.end(), [&](int p, int q) {
+      auto kp = tkey(p), kq = tkey(q);
+      return kp != kq ? kp < kq : p < q;
+    });
+    auto free_nbrs = [&](int t) {
+      int c = 0;
+      for (int e = 0; e < 3; ++e) {
+        int u = tnbr(t, e);
+        if (u != t && mate[u] < 0) ++c;
+      }
+      return c;
+    };
+    for (int t : order) {
+      if (mate[t] >= 0) continue;
+      int best = -1, bestc = 99;
+      for (int e = 0; e < 3; ++e) {
+        int u = tnbr(t, e);
+        if (u == t || mate[u] >= 0) continue;
+        mate[t] = t;   // count u's free neighbours without t
+        int c = free_nbrs(u);
+        mate[t] = -1;
+        if (c < bestc) { bestc = c; best = u; }
+      }
+      if (best >= 0) { mate[t] = best; mate[best] = t; }
+    }
+    // augmenting paths (alternating BFS without blossom handling: a heuristic that only ever
+    // increases the matching; correctness does not depend on it being maximum)
+    for (int root : order) {
+      if (mate[root] >= 0) continue;
+      std::vector<int> parent(T, -1), seen(T, 0);
+      std::deque<int> q;
+      q.push_back(root);
+      seen[root] = 1;
+      int found = -1;
+      while (!q.empty() && found < 0) {
+        int t = q.front();
+        q.pop_front();
+        for (int e = 0; e < 3 && found < 0; ++e) {
+          int u = tnbr(t, e);
+          if (u == t || seen[u]) continue;
+          seen[u] = 1;
+          parent[u] = t;
+          if (mate[u] < 0) { found = u; break; }
+          int w = mate[u];
+          if (!seen[w]) { seen[w] = 1; parent[w] = u; q.push_back(w); }
+        }
+      }
+      if (found < 0) continue;
+      // flip along the path found <- parent ... <- root
+      int u = found;
+      while (u != root) {
+        int t = parent[u];          // t is an "even" vertex: (t,u) becomes matched
+        int prev = mate[t];         // t's old mate (or -1 for the root)
+        mate[t] = u; mate[u] = t;
+        if (t == root) break;
+        u = prev;                   // prev's new partner is parent[prev]... continue flipping
+        mate[u] = -1;
+      }
+    }
+    // sanity: mate must be an involution
+    for (int t = 0; t < T; ++t)
+      if (mate[t] >= 0 && (mate[t] == t || mate[mate[t]] != t)) {
+        for (int q2 = 0; q2 < T; ++q2) mate[q2] = -1;   // give up pairing: all single triangles
+        break;
+      }
+  }
+
+  // ---- element constants.  dminv of a triangle for an arbitrary cyclic vertex order (p0,p1,p2):
+  //      frame t1 = e1/|e1|, t2 = n x t1, D_m = [[|e1|, e2.t1], [0, e2.t2]]  (same construction as
+  //      tri_dminv above; a cyclic shift only rotates F on the right, which no energy sees).
+  auto dminv_of = [&](int p0, int p1, int p2, double out3[3]) {
+    V3 a = Xv(p0), b = Xv(p1), c = Xv(p2);
+    V3 e1 = b - a, e2 = c - a;
+    double twoA = norm(cross(e1, e2)), l1 = norm(e1);
+    double d00 = l1, d01 = dot(e2, e1) / l1, d11 = twoA / l1;
+    out3[0] = 1.0 / d00;
+    out3[1] = -d01 / (d00 * d11);
+    out3[2] = 1.0 / d11;
+  };
+  // hinge on the undirected edge (p,q) seen from the element whose own opposite vertex is oo
+  auto hinge_consts = [&](int p, int q, int oo, float out4[4]) {
+    int hh = hinge_of[(size_t)p * n + q];
+    const int32_t* hv = &P->hinge_verts[4 * (size_t)hh];
+    const double* K = &P->hinge_K[4 * (size_t)hh];
+    double sw = std::sqrt(P->hinge_wr[2 * (size_t)hh]);
+    auto Kof = [&](int vtx) {
+      for (int i = 0; i < 4; ++i)
+        if (hv[i] == vtx) return K[i];
+      return 0.0;
+    };
+    out4[0] = (float)(sw * Kof(p));
+    out4[1] = (float)(sw * Kof(q));
+    out4[2] = (float)(sw * Kof(oo));
+    out4[3] = (float)(sw * P->hinge_wr[2 * (size_t)hh + 1]);
+  };
+  struct Proto { int t1, t2, a, b, c, d; };
+  std::vector<Proto> protos;
+  {
+    std::vector<uint8_t> done(T, 0);
+    for (int t = 0; t < T; ++t) {
+      if (done[t]) continue;
+      done[t] = 1;
+      Proto pr{};
+      pr.t1 = t;
+      int eshared = 0;
+      if (mate[t] >= 0) {
+        for (int e = 0; e < 3; ++e)
+          if (tnbr(t, e) == mate[t]) { eshared = e; break; }
+        pr.t2 = mate[t];
+        done[mate[t]] = 1;
+      } else {
+        pr.t2 = -1;
+      }
+      pr.a = tris[3 * t + eshared];
+      pr.b = tris[3 * t + (eshared + 1) % 3];
+      pr.c = tris[3 * t + (eshared + 2) % 3];
+      pr.d = opposite(pr.b, pr.a);
+      protos.push_back(pr);
     }
   }
+  // element order: by smallest internal vertex id, then by the id sum (locality in shared memory)
+  std::sort(protos.begin(), protos.end(), [&](const Proto& x, const Proto& y) {
+    auto key = [&](const Proto& p) {
+      int a = P->iperm[p.a], b = P->iperm[p.b], c = P->iperm[p.c];
+      return std::make_pair(std::min(a, std::min(b, c)), a + b + c);
+    };
+    auto kx = key(x), ky = key(y);
+    return kx != ky ? kx < ky : x.t1 < y.t1;
+  });
+  const int E = (int)protos.size();
+  if (E > 1024) return fail(NPFEM_ELIMIT, "mesh needs more than 1024 elements per cell");
+  P->E = E;
+  P->n_diamonds = 0;
+  P->elem.assign(E, ElemConst{});
+  P->elem_tris.assign(2 * (size_t)E, -1);
+  std::vector<std::vector<uint16_t>> inc(n);   // per internal vertex: out-slot byte offsets
+  for (int e = 0; e < E; ++e) {
+    const Proto& pr = protos[e];
+    ElemConst& ec = P->elem[e];
+    const bool diamond = pr.t2 >= 0;
+    P->n_diamonds += diamond ? 1 : 0;
+    P->elem_tris[2 * (size_t)e] = pr.t1;
+    P->elem_tris[2 * (size_t)e + 1] = pr.t2;
+    const int a = pr.a, b = pr.b, c = pr.c, d = pr.d;
+    const int f1 = opposite(c, b), f2 = opposite(a, c);
+    const int f3 = diamond ? opposite(d, a) : a, f4 = diamond ? opposite(b, d) : a;
+    const int idv[8] = {a, b, c, d, f1, f2, f3, f4};
+    for (int s = 0; s < 8; ++s) ec.ids[s] = (uint16_t)P->iperm[idv[s]];
+    double dm[3];
+    dminv_of(a, b, c, dm);
+    ec.f[0] = (float)dm[0]; ec.f[1] = (float)dm[1]; ec.f[2] = (float)dm[2];
+    ec.f[3] = (float)(mat->k_strain * P->tri_area[pr.t1]);
+    ec.f[4] = (float)(mat->k_area * P->tri_area[pr.t1]);
+    dminv_of(b, a, d, dm);   // the real neighbour triangle even for a single: finite arithmetic
+    ec.f[5] = (float)dm[0]; ec.f[6] = (float)dm[1]; ec.f[7] = (float)dm[2];
+    ec.f[8] = diamond ? (float)(mat->k_strain * P->tri_area[pr.t2]) : 0.0f;
+    ec.f[9] = diamond ? (float)(mat->k_area * P->tri_area[pr.t2]) : 0.0f;
+    hinge_consts(a, b, c, &ec.f[10]);
+    hinge_consts(b, c, a, &ec.f[14]);
+    hinge_consts(c, a, b, &ec.f[18]);
+    if (diamond) {
+      hinge_consts(a, d, b, &ec.f[22]);
+      hinge_consts(d, b, a, &ec.f[26]);
+    } else {
+      for (int q = 22; q < 30; ++q) ec.f[q] = 0.0f;
+    }
+    ec.f[30] = diamond ? 1.0f : 0.5f;
+    const int nslots = diamond ? 4 : 3;
+    for (int s = 0; s < nslots; ++s)
+      inc[P->iperm[idv[s]]].push_back((uint16_t)((e * 4 + s) * 16));
+  }
   P->inc_ptr.assign(n + 1, 0);
-  P->inc_out.clear();
-  P->inc_ring.clear();
+  P->inc_off.clear();
+  for (int i = 0; i < n; ++i) {
+    for (uint16_t o16 : inc[i]) P->inc_off.push_back(o16);
+    P->inc_ptr[i + 1] = (uint16_t)P->inc_off.size();
+  }
+
+  // ---- ring neighbours of every vertex in cyclic (counter-clockwise seen from outside) order:
+  //      triangle i of the fan is (v, r_i, r_i+1); grad V at v = 1/6 sum_i (r_i - v) x (r_i+1 - v)
+  P->ring_ptr.assign(n + 1, 0);
+  P->ring_off.clear();
   for (int i = 0; i < n; ++i) {
     int ve = P->perm[i];
     int t0 = -1, s0 = 0;
@@ -435,8 +599,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     int t = t0, s = s0, count = 0;
     do {
       int r0 = tris[3 * t + (s + 1) % 3], r1 = tris[3 * t + (s + 2) % 3];
-      P->inc_out.push_back((uint16_t)(tint[t] * 9 + s * 3));
-      P->inc_ring.push_back((uint16_t)P->iperm[r0]);
+      P->ring_off.push_back((uint16_t)(P->iperm[r0] * 16));
       // next triangle around ve holds the directed edge ve -> r1
       int tn = etri[(size_t)ve * n + r1];
       s = eslot[(size_t)ve * n + r1];
@@ -444,23 +607,23 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
       if (++count > T) return fail(NPFEM_EINVAL, "non-manifold vertex fan");
     } while (t != t0);
     if (count != (int)adj[ve].size()) return fail(NPFEM_EINVAL, "non-manifold vertex (several fans)");
-    P->inc_ptr[i + 1] = (uint16_t)P->inc_out.size();
+    P->ring_ptr[i + 1] = (uint16_t)P->ring_off.size();
   }
 
-  // ---- launch configuration
-  int need = std::max(n, (T + kTrisPerThread - 1) / kTrisPerThread);
+  // ---- launch configuration: one thread per element and per (padded) vertex
+  int need = std::max(nvb * 8, E);
   P->threads = (need + 31) / 32 * 32;
   if (P->threads > 1024) return fail(NPFEM_ELIMIT, "mesh needs more than 1024 threads per cell");
   const int smem_max = kSmemMaxDynamic;
   int k = o.cells_per_cta ? o.cells_per_cta : kMaxCellsPerCta;
-  while (k > 1 && smem_layout(n, T, nvb, k).total > smem_max) {
+  while (k > 1 && smem_layout(n, E, nvb, k).total > smem_max) {
     if (o.cells_per_cta) return fail(NPFEM_ELIMIT, "requested cells_per_cta does not fit shared memory");
     --k;
   }
-  if (smem_layout(n, T, nvb, k).total > smem_max)
+  if (smem_layout(n, E, nvb, k).total > smem_max)
     return fail(NPFEM_ELIMIT, "cell state does not fit the shared memory of one SM");
   P->cells_per_cta = k;
-  P->smem_bytes = smem_layout(n, T, nvb, k).total;
+  P->smem_bytes = smem_layout(n, E, nvb, k).total;
   P->global_mode = o.global_mode ? o.global_mode : 2;
   o.cells_per_cta = k;
   o.global_mode = P->global_mode;
