@@ -180,23 +180,31 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   // ---- one blob for all constant tables, 256-byte aligned sections
   const int n = P.n, E = P.E, NP = P.nvb * 8;
   std::vector<uint16_t> perm16(NP, 0);
-  std::vector<uint32_t> elem_ids(4 * (size_t)E);
-  std::vector<float> elem_f((size_t)kElemFloats * E), h2m(NP, 0.0f), mh2(NP, 0.0f);
+  // element constants as kElemGroups groups of 4 words, group-major ([group][E] float4):
+  //   0: packed byte offsets 16*id of (a,b) (c,d) (f1,f2) (f3,f4)   1: t1 i00 i01 i11 w_s
+  //   2: t2 i00 i01 i11 w_s      3: t1 w_a, t2 w_a, he, 0           4..8: hinge e: Kp Kq Ko r'
+  std::vector<uint32_t> elem_c((size_t)kElemGroups * E * 4, 0u);
+  std::vector<float> h2m(NP, 0.0f), mh2(NP, 0.0f);
   for (int i = 0; i < n; ++i) {
     perm16[i] = (uint16_t)P.perm[i];
     h2m[i] = P.h2_over_m[i];
     mh2[i] = P.m_over_h2[i];
   }
+  auto fbits = [](float x) { uint32_t u; std::memcpy(&u, &x, 4); return u; };
   for (int e = 0; e < E; ++e) {
     const ElemConst& ec = P.elem[e];
-    for (int q = 0; q < 4; ++q)   // byte offsets of the float4 positions: 16 * internal id
-      elem_ids[(size_t)q * E + e] = (uint32_t)ec.ids[2 * q] * 16u | ((uint32_t)ec.ids[2 * q + 1] * 16u) << 16;
-    for (int q = 0; q < kElemFloats; ++q) elem_f[(size_t)q * E + e] = ec.f[q];
+    auto W = [&](int g, int w) -> uint32_t& { return elem_c[((size_t)g * E + e) * 4 + w]; };
+    for (int q = 0; q < 4; ++q)
+      W(0, q) = (uint32_t)ec.ids[2 * q] * 16u | ((uint32_t)ec.ids[2 * q + 1] * 16u) << 16;
+    for (int q = 0; q < 4; ++q) { W(1, q) = fbits(ec.f[q]); W(2, q) = fbits(ec.f[5 + q]); }
+    W(3, 0) = fbits(ec.f[4]); W(3, 1) = fbits(ec.f[9]); W(3, 2) = fbits(ec.f[30]);
+    for (int hgi = 0; hgi < 5; ++hgi)
+      for (int q = 0; q < 4; ++q) W(4 + hgi, q) = fbits(ec.f[10 + 4 * hgi + q]);
   }
   struct Sec { const void* src; size_t bytes; size_t off; };
   Sec secs[] = {
-      {perm16.data(), perm16.size() * 2, 0},          {elem_ids.data(), elem_ids.size() * 4, 0},
-      {elem_f.data(), elem_f.size() * 4, 0},          {h2m.data(), h2m.size() * 4, 0},
+      {perm16.data(), perm16.size() * 2, 0},          {elem_c.data(), elem_c.size() * 4, 0},
+      {nullptr, 0, 0},                                {h2m.data(), h2m.size() * 4, 0},
       {mh2.data(), mh2.size() * 4, 0},                {P.inc_ptr.data(), P.inc_ptr.size() * 2, 0},
       {P.inc_off.data(), P.inc_off.size() * 2, 0},    {P.ring_ptr.data(), P.ring_ptr.size() * 2, 0},
       {P.ring_off.data(), P.ring_off.size() * 2, 0},  {P.blk_ptr.data(), P.blk_ptr.size() * 4, 0},
@@ -207,6 +215,7 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   e = cudaMalloc(&H->blob, total);
   if (e != cudaSuccess) { delete H; return cuda_err(e, "cudaMalloc(constants)"); }
   for (auto& sct : secs) {
+    if (!sct.bytes) continue;
     e = cudaMemcpy(static_cast<char*>(H->blob) + sct.off, sct.src, sct.bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(H->blob); delete H; return cuda_err(e, "cudaMemcpy(constants)"); }
   }
@@ -219,8 +228,7 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.s_min = (float)P.mat.s_min; D.s_max = (float)P.mat.s_max;
   D.a_min = (float)P.mat.a_min; D.a_max = (float)P.mat.a_max;
   D.perm = reinterpret_cast<const uint16_t*>(base + secs[0].off);
-  D.elem_ids = reinterpret_cast<const uint32_t*>(base + secs[1].off);
-  D.elem_f = reinterpret_cast<const float*>(base + secs[2].off);
+  D.elem_c = reinterpret_cast<const float4*>(base + secs[1].off);
   D.h2_over_m = reinterpret_cast<const float*>(base + secs[3].off);
   D.m_over_h2 = reinterpret_cast<const float*>(base + secs[4].off);
   D.inc_ptr = reinterpret_cast<const uint16_t*>(base + secs[5].off);

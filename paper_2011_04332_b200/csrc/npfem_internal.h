@@ -85,14 +85,17 @@ int build_plan(int n_verts, int n_tris, const int32_t* tris, const double* rest_
 
 // Shared-memory carve-up used by both the host (to size the launch) and the kernel.
 //   z4   [k][NP] float4   current iterate z = s + d, cell-local coordinates (w unused)
-//   s, d [3k][NP] float   inertial prediction and correction, row m = 3*cell + component
+//   ec   [9][E] float4    element constants (kElemGroups groups of 4 words, see npfem_api.cu)
 //   ra   [nvb][32] float4 right-hand sides in mma A-fragment order (fp32 while the local step
 //                         accumulates them, then their tf32 high parts)
-//   rb   max(E*64, NP*64) element results `out` [E][4] float4 during the local step, then the
-//                         tf32 low parts of the right-hand sides during the global step
+//   rb   max(E*64, NP*64) element results `out` [4][E] float4 during the local step, then the
+//                         tf32 low parts of the right-hand sides, then the increments of d
 //   red  [5][32] float4   per-warp partial sums of the volume reductions
+// The inertial prediction s and the correction d are private to the thread that owns the vertex
+// and live in tensor memory (TMEM), 32 columns per group of 4 warps.
+constexpr int kElemGroups = 9;
 struct SmemLayout {
-  int z4, s, d, ra, rb, red, total;   // byte offsets
+  int z4, ec, ra, rb, red, total;   // byte offsets
 };
 inline SmemLayout smem_layout(int n, int E, int nvb, int k) {
   (void)n;
@@ -100,8 +103,7 @@ inline SmemLayout smem_layout(int n, int E, int nvb, int k) {
   SmemLayout L{};
   int off = 0;
   L.z4 = off; off += k * NP * 16;
-  L.s = off; off += 3 * k * NP * 4;
-  L.d = off; off += 3 * k * NP * 4;
+  L.ec = off; off += kElemGroups * E * 16;
   L.ra = off; off += NP * 64;
   int rb = E * 64 > NP * 64 ? E * 64 : NP * 64;
   L.rb = off; off += rb;

@@ -16,10 +16,11 @@
 // lineage), but never differences world coordinates.
 //
 // Work mapping per iteration and cell: thread e < E owns one ELEMENT (two triangles sharing an
-// edge, npfem_internal.h) and writes one float4 per own vertex; thread v < n owns one VERTEX,
-// gathers its element slots, evaluates grad V on its ring and forms the right-hand side; the
-// global step then multiplies all 16 right-hand-side columns of the CTA by the block-sparse
-// inverse on the tensor cores (3xTF32 split, fp32 accumulate).
+// edge, npfem_internal.h; its constants are staged once in shared memory) and writes one float4
+// per own vertex; thread v < n owns one VERTEX, gathers its element slots, evaluates grad V on
+// its ring and forms the right-hand side; the global step then multiplies all 16 right-hand-side
+// columns of the CTA by the block-sparse inverse on the tensor cores (3xTF32 split, fp32
+// accumulate).  s and d, private to the owner thread, live in tensor memory (TMEM).
 #include <cstdint>
 
 #include "npfem_kernels.cuh"
@@ -79,13 +80,15 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
+
 // Closest point of the hyperbola branch {t1*t2 = q^2, t > 0} to (s1, s2), s1 >= s2 > 0, written
 // as (q p, q / p) with p >= 1: root of  g(p) = q p^4 - s1 p^3 + s2 p - q  (stationarity of the
-// squared distance), bracketed in [1, max(s1/q, q/s2)] where g changes sign from <= 0 to >= 0.
-// Newton from the same-ratio point sqrt(s1/s2), bisection whenever Newton leaves the bracket.
-__device__ __forceinline__ float hyperbola_p(float s1, float s2, float q) {
+// squared distance).  Start: the same-ratio point p0 = sqrt(s1/s2), where g(p0) = (p0^4 - 1)
+// (q - sqrt(s1 s2)) is already small for nearly isotropic or nearly area-preserving states.
+// Safeguarded variant: bracket [1, max(s1/q, q/s2)] (g goes from <= 0 to >= 0), Newton with
+// bisection whenever Newton leaves the bracket.
+__device__ __noinline__ float hyperbola_p_safe(float s1, float s2, float q, float p) {
   float lo = 1.0f, hi = fmaxf(fdiv(s1, q), fdiv(q, s2));
-  float p = fsqrt(fdiv(s1, s2));
   p = fminf(fmaxf(p, lo), hi);
   for (int it = 0; it < 24; ++it) {
     float p2 = p * p;
@@ -99,6 +102,23 @@ __device__ __forceinline__ float hyperbola_p(float s1, float s2, float q) {
     if (step <= 2.4e-7f * p) break;
   }
   return p;
+}
+// Fast variant for moderate deformations (s1/s2 < 1.5 and |s1 s2 - q^2| < 0.4 q^2): three plain
+// Newton steps from p0, quadratically convergent there (start error < 0.1 => < 1e-7 after 3).
+__device__ __forceinline__ float hyperbola_p(float s1, float s2, float q, float ratio, float J) {
+  float p = fsqrt(ratio);
+  const float q2 = q * q;
+  if (ratio < 1.5f && fabsf(J - q2) < 0.4f * q2) {
+#pragma unroll
+    for (int it = 0; it < 3; ++it) {
+      const float p2 = p * p;
+      const float g = fmaf(fmaf(q, p, -s1), p2 * p, fmaf(s2, p, -q));
+      const float dg = fmaf(fmaf(4.0f * q, p, -3.0f * s1), p2, s2);
+      p = fmaf(-g, frcp(dg), p);
+    }
+    return p;
+  }
+  return hyperbola_p_safe(s1, s2, q, p);
 }
 
 // Membrane part of the local step for one triangle (p0,p1,p2) with edges e1 = z1 - z0,
@@ -116,22 +136,23 @@ __device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, flo
   const float tau = fsqrt(C11 + C22 + 2.0f * J);              // sigma1 + sigma2
   const float dC = C11 - C22;
   const float Delta = fsqrt(fmaf(dC, dC, 4.0f * C12 * C12));  // sigma1^2 - sigma2^2
-  const float delta = fdiv(Delta, fmaxf(tau, 1e-30f));        // sigma1 - sigma2
+  const float delta = Delta * frcp(fmaxf(tau, 1e-30f));       // sigma1 - sigma2
   const float s1 = 0.5f * (tau + delta);
   const float s2 = fmaxf(0.5f * (tau - delta), 1e-30f);
   // g_i = sum_terms w (projected sigma_i - sigma_i) / sigma_i   (residual form: P - F = F V diag(g) V^T)
-  const float r1 = frcp(s1), r2 = frcp(s2);
+  const float rJ = frcp(fmaxf(s1 * s2, 1e-30f));
+  const float r1 = s2 * rJ, r2 = s1 * rJ;                     // 1/sigma1, 1/sigma2
   float g1 = ws * (fminf(fmaxf(s1, P.s_min), P.s_max) - s1) * r1;
   float g2 = ws * (fminf(fmaxf(s2, P.s_min), P.s_max) - s2) * r2;
   const float astar = fminf(fmaxf(J, P.a_min), P.a_max);
   if (J != astar) {
     const float q = fsqrt(astar);
-    const float p = hyperbola_p(s1, s2, q);
-    g1 = fmaf(wa, (q * p - s1) * r1, g1);
-    g2 = fmaf(wa, (fdiv(q, p) - s2) * r2, g2);
+    const float p = hyperbola_p(s1, s2, q, s1 * r2, J);
+    g1 = fmaf(wa, fmaf(q, p, -s1) * r1, g1);
+    g2 = fmaf(wa, fmaf(q, frcp(p), -s2) * r2, g2);
   }
   const float gbar = 0.5f * (g1 + g2);
-  const float rho = fdiv(g1 - g2, fmaxf(Delta, 1e-30f));
+  const float rho = (g1 - g2) * frcp(fmaxf(Delta, 1e-30f));
   const float S00 = fmaf(rho, 0.5f * dC, gbar), S11 = fmaf(-rho, 0.5f * dC, gbar), S01 = rho * C12;
   const F3 Q0 = fma3(S00, F0, S01 * F1);
   const F3 Q1 = fma3(S01, F0, S11 * F1);
@@ -157,25 +178,45 @@ __device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], 
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
 }
 
-// Register-resident constants of one element (npfem_internal.h: ElemConst).
-struct ElemReg {
-  uint32_t ab, cd, f12, f34;   // packed byte offsets (16 * internal id) into a cell's z4
-  float f[kElemFloats];
-};
+// ---- tensor memory as per-thread scratch: thread (warp w, lane l) owns TMEM lane 32*(w%4) + l;
+//      a 32x32b.x16 access moves 16 consecutive columns of that lane to / from 16 registers.
+__device__ __forceinline__ void tmem_st16(uint32_t a, const float (&v)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+      :: "r"(a), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]),
+         "f"(v[8]), "f"(v[9]), "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
+      : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]),
+        "=f"(v[8]), "=f"(v[9]), "=f"(v[10]), "=f"(v[11]), "=f"(v[12]), "=f"(v[13]), "=f"(v[14]), "=f"(v[15])
+      : "r"(a)
+      : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
 
 // Local step of one element for one cell: membrane residuals of its two triangles and the five
-// hinges it sees, summed per own vertex (a,b,c,d) into out4[0..3].  zc = the cell's z4 array.
-__device__ __forceinline__ void element_residual(const ElemReg& er, const unsigned char* __restrict__ zc,
+// hinges it sees, summed per own vertex (a,b,c,d) into out4[slot * E].  ec = the element's
+// constants in shared memory (group g at ec[g * E], npfem_api.cu), zc = the cell's z4 array.
+__device__ __forceinline__ void element_residual(const float4* __restrict__ ec, int E,
+                                                 const unsigned char* __restrict__ zc,
                                                  const DevParams& P, float4* __restrict__ out4) {
-  const F3 za = lds3(zc, er.ab & 0xffffu), zb = lds3(zc, er.ab >> 16);
-  const F3 zc3 = lds3(zc, er.cd & 0xffffu), zd = lds3(zc, er.cd >> 16);
+  const float4 idw = ec[0];
+  const uint32_t id_ab = __float_as_uint(idw.x), id_cd = __float_as_uint(idw.y);
+  const uint32_t id_f12 = __float_as_uint(idw.z), id_f34 = __float_as_uint(idw.w);
+  const F3 za = lds3(zc, id_ab & 0xffffu), zb = lds3(zc, id_ab >> 16);
+  const F3 zc3 = lds3(zc, id_cd & 0xffffu), zd = lds3(zc, id_cd >> 16);
   const F3 eab = zb - za, eac = zc3 - za, ebc = zc3 - zb, ead = zd - za, ebd = zd - zb;
   const F3 eba = {-eab.x, -eab.y, -eab.z};
 
   // ---- membranes: t1 = (a,b,c) from a; t2 = (b,a,d) from b
+  const float4 m1 = ec[E], m2 = ec[2 * E], m3 = ec[3 * E];
   F3 t1b, t1c, t2a, t2d;
-  membrane(eab, eac, er.f[0], er.f[1], er.f[2], er.f[3], er.f[4], P, t1b, t1c);
-  membrane(eba, ebd, er.f[5], er.f[6], er.f[7], er.f[8], er.f[9], P, t2a, t2d);
+  membrane(eab, eac, m1.x, m1.y, m1.z, m1.w, m3.x, P, t1b, t1c);
+  membrane(eba, ebd, m2.x, m2.y, m2.z, m2.w, m3.y, P, t2a, t2d);
   F3 fa = t2a - (t1b + t1c);
   F3 fb = t1b - (t2a + t2d);
   F3 fc = t1c;
@@ -183,50 +224,51 @@ __device__ __forceinline__ void element_residual(const ElemReg& er, const unsign
 
   // ---- shared hinge (a,b | c ; d): once in full for a diamond, the element's half for a single
   {
-    const float Kp = er.f[10], Kq = er.f[11], Ko = er.f[12];
-    const float Kf = -(Kp + Kq + Ko), he = er.f[30], hf = fmaf(2.0f, he, -1.0f);
-    const F3 kv = hinge_vec(Kq, Ko, Kf, er.f[13], eab, eac, ead);
+    const float4 hk = ec[4 * E];
+    const float Kp = hk.x, Kq = hk.y, Ko = hk.z;
+    const float Kf = -(Kp + Kq + Ko), he = m3.z, hf = fmaf(2.0f, he, -1.0f);
+    const F3 kv = hinge_vec(Kq, Ko, Kf, hk.w, eab, eac, ead);
     fa = fma3(he * Kp, kv, fa); fb = fma3(he * Kq, kv, fb);
     fc = fma3(Ko, kv, fc);      fd = fma3(hf * Kf, kv, fd);
   }
   // ---- outer hinges: half of the end-point terms, all of the own opposite vertex's term
   {   // (b,c | a ; f1)
-    const float Kp = er.f[14], Kq = er.f[15], Ko = er.f[16];
-    const F3 zf = lds3(zc, er.f12 & 0xffffu);
-    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[17], ebc, eba, zf - zb);
-    fb = fma3(0.5f * Kp, kv, fb); fc = fma3(0.5f * Kq, kv, fc); fa = fma3(Ko, kv, fa);
+    const float4 hk = ec[5 * E];
+    const F3 zf = lds3(zc, id_f12 & 0xffffu);
+    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, ebc, eba, zf - zb);
+    fb = fma3(0.5f * hk.x, kv, fb); fc = fma3(0.5f * hk.y, kv, fc); fa = fma3(hk.z, kv, fa);
   }
   {   // (c,a | b ; f2)
-    const float Kp = er.f[18], Kq = er.f[19], Ko = er.f[20];
-    const F3 zf = lds3(zc, er.f12 >> 16);
+    const float4 hk = ec[6 * E];
+    const F3 zf = lds3(zc, id_f12 >> 16);
     const F3 eca = {-eac.x, -eac.y, -eac.z}, ecb = {-ebc.x, -ebc.y, -ebc.z};
-    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[21], eca, ecb, zf - zc3);
-    fc = fma3(0.5f * Kp, kv, fc); fa = fma3(0.5f * Kq, kv, fa); fb = fma3(Ko, kv, fb);
+    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, eca, ecb, zf - zc3);
+    fc = fma3(0.5f * hk.x, kv, fc); fa = fma3(0.5f * hk.y, kv, fa); fb = fma3(hk.z, kv, fb);
   }
   {   // (a,d | b ; f3)
-    const float Kp = er.f[22], Kq = er.f[23], Ko = er.f[24];
-    const F3 zf = lds3(zc, er.f34 & 0xffffu);
-    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[25], ead, eab, zf - za);
-    fa = fma3(0.5f * Kp, kv, fa); fd = fma3(0.5f * Kq, kv, fd); fb = fma3(Ko, kv, fb);
+    const float4 hk = ec[7 * E];
+    const F3 zf = lds3(zc, id_f34 & 0xffffu);
+    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, ead, eab, zf - za);
+    fa = fma3(0.5f * hk.x, kv, fa); fd = fma3(0.5f * hk.y, kv, fd); fb = fma3(hk.z, kv, fb);
   }
   {   // (d,b | a ; f4)
-    const float Kp = er.f[26], Kq = er.f[27], Ko = er.f[28];
-    const F3 zf = lds3(zc, er.f34 >> 16);
+    const float4 hk = ec[8 * E];
+    const F3 zf = lds3(zc, id_f34 >> 16);
     const F3 edb = {-ebd.x, -ebd.y, -ebd.z}, eda = {-ead.x, -ead.y, -ead.z};
-    const F3 kv = hinge_vec(Kq, Ko, -(Kp + Kq + Ko), er.f[29], edb, eda, zf - zd);
-    fd = fma3(0.5f * Kp, kv, fd); fb = fma3(0.5f * Kq, kv, fb); fa = fma3(Ko, kv, fa);
+    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, edb, eda, zf - zd);
+    fd = fma3(0.5f * hk.x, kv, fd); fb = fma3(0.5f * hk.y, kv, fb); fa = fma3(hk.z, kv, fa);
   }
   out4[0] = make_float4(fa.x, fa.y, fa.z, 0.0f);
-  out4[1] = make_float4(fb.x, fb.y, fb.z, 0.0f);
-  out4[2] = make_float4(fc.x, fc.y, fc.z, 0.0f);
-  out4[3] = make_float4(fd.x, fd.y, fd.z, 0.0f);
+  out4[E] = make_float4(fb.x, fb.y, fb.z, 0.0f);
+  out4[2 * E] = make_float4(fc.x, fc.y, fc.z, 0.0f);
+  out4[3 * E] = make_float4(fd.x, fd.y, fd.z, 0.0f);
 }
 
 // grad V at a vertex = 1/6 sum over its fan of (r_i - z) x (r_i+1 - z); the first kRegList ring
 // offsets come from registers, longer fans continue from the global list.
 __device__ __forceinline__ F3 ring_gradient(const unsigned char* zc, F3 zv, int rcnt,
                                             const uint32_t (&roff)[kRegList / 2],
-                                            const uint16_t* __restrict__ ring_tail) {
+                                            const DevParams& P, int v) {
   const F3 e0 = lds3(zc, roff[0] & 0xffffu) - zv;
   F3 ep = e0, g = {0.f, 0.f, 0.f};
 #pragma unroll
@@ -237,10 +279,13 @@ __device__ __forceinline__ F3 ring_gradient(const unsigned char* zc, F3 zv, int 
       ep = e;
     }
   }
-  for (int i = kRegList; i < rcnt; ++i) {
-    const F3 e = lds3(zc, ring_tail[i]) - zv;
-    g = cross_acc(ep, e, g);
-    ep = e;
+  if (rcnt > kRegList) {
+    const uint16_t* ring_tail = P.ring_off + P.ring_ptr[v];
+    for (int i = kRegList; i < rcnt; ++i) {
+      const F3 e = lds3(zc, ring_tail[i]) - zv;
+      g = cross_acc(ep, e, g);
+      ep = e;
+    }
   }
   g = cross_acc(ep, e0, g);
   return (1.0f / 6.0f) * g;
@@ -253,13 +298,13 @@ __device__ __forceinline__ F3 ring_gradient(const unsigned char* zc, F3 zv, int 
 template <int MODE, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  unsigned char* const z4b = smem_raw + P.L.z4;                       // [k][NP] float4 iterate z
-  float* const s = reinterpret_cast<float*>(smem_raw + P.L.s);        // [3k][NP] inertial prediction
-  float* const d = reinterpret_cast<float*>(smem_raw + P.L.d);        // [3k][NP] correction d^k
-  float* const ra = reinterpret_cast<float*>(smem_raw + P.L.ra);      // rhs, A-fragment order (fp32 / hi)
-  unsigned char* const rbb = smem_raw + P.L.rb;                       // element results / rhs lo parts
+  unsigned char* const z4b = smem_raw + P.L.z4;                        // [k][NP] float4 iterate z
+  const float4* const ecs = reinterpret_cast<const float4*>(smem_raw + P.L.ec);   // element constants
+  float* const ra = reinterpret_cast<float*>(smem_raw + P.L.ra);       // rhs, A-fragment order (fp32 / hi)
+  unsigned char* const rbb = smem_raw + P.L.rb;                        // element results / rhs lo / delta d
   float* const rb = reinterpret_cast<float*>(rbb);
-  float4* const red = reinterpret_cast<float4*>(smem_raw + P.L.red);  // [k][32] partial sums
+  float4* const red = reinterpret_cast<float4*>(smem_raw + P.L.red);   // [5][32] partial sums
+  __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
   const int n = P.n, E = P.E, nvb = P.nvb, NP = nvb * 8;
@@ -267,33 +312,29 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const int kact = min(P.k, P.n_cells - cell0);
   const int cellz = NP * 16;                      // bytes of one cell's z4
 
-  // ---- per-thread constants: one element and one vertex
-  const bool is_e = tid < E, isv = tid < n, isvp = tid < NP;
-  ElemReg er;
-  {
-    const int e = is_e ? tid : 0;
-    er.ab = P.elem_ids[e]; er.cd = P.elem_ids[E + e];
-    er.f12 = P.elem_ids[2 * E + e]; er.f34 = P.elem_ids[3 * E + e];
-#pragma unroll
-    for (int q = 0; q < kElemFloats; ++q) er.f[q] = P.elem_f[q * E + e];
+  // ---- tensor memory: 32 columns (s: 0..14, d: 16..30) per group of 4 warps
+  uint32_t tmem_cols = 32;
+  while (tmem_cols < 32u * ((nwarps + 3) >> 2)) tmem_cols <<= 1;
+  if (warp == 0) {
+    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(sa), "r"(tmem_cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
+
+  // ---- per-thread constants of the vertex role
+  const bool is_e = tid < E, isv = tid < n, isvp = tid < NP;
   const int v = isvp ? tid : 0;
-  const int vext = P.perm[v];
-  const float h2m = P.h2_over_m[v], mh2 = P.m_over_h2[v];
+  const float mh2 = P.m_over_h2[v];
   const float h = P.h;
   int icnt = 0, rcnt = 0;
   uint32_t ioff[kRegList / 2] = {0, 0, 0}, roff[kRegList / 2] = {0, 0, 0};
-  const uint16_t* inc_tail = P.inc_off;
-  const uint16_t* ring_tail = P.ring_off;
   if (isv) {
     const int i0 = P.inc_ptr[v], r0 = P.ring_ptr[v];
     icnt = P.inc_ptr[v + 1] - i0;
     rcnt = P.ring_ptr[v + 1] - r0;
-    inc_tail += i0;
-    ring_tail += r0;
 #pragma unroll
     for (int i = 0; i < kRegList; ++i) {
-      const uint32_t io = i < icnt ? inc_tail[i] : 0u, ro = i < rcnt ? ring_tail[i] : 0u;
+      const uint32_t io = i < icnt ? P.inc_off[i0 + i] : 0u, ro = i < rcnt ? P.ring_off[r0 + i] : 0u;
       ioff[i >> 1] |= io << (16 * (i & 1));
       roff[i >> 1] |= ro << (16 * (i & 1));
     }
@@ -302,14 +343,22 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   //   block jb = v/8 holds 32 lanes x float4; lane = (m&7)*4 + (v&3), component = 2*((v&7)>>2) + (m>>3)
   const int fbase = ((v >> 3) * 32 + (v & 3)) * 4 + 2 * ((v & 7) >> 2);
 
-  // ---- zero the state that padding vertices / missing cells never write
+  // ---- stage the element constants; zero what padding vertices / missing cells never write
+  for (int i = tid; i < kElemGroups * E; i += blockDim.x)
+    reinterpret_cast<float4*>(smem_raw + P.L.ec)[i] = P.elem_c[i];
   for (int i = tid; i < NP * 16; i += blockDim.x) ra[i] = 0.0f;
-  for (int i = tid; i < 3 * P.k * NP; i += blockDim.x) { s[i] = 0.0f; d[i] = 0.0f; }
   for (int i = tid; i < P.k * NP; i += blockDim.x)
     reinterpret_cast<float4*>(z4b)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t ta = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 32);
+
   // ---- prologue: load state, centroid, local coordinates, inertial prediction
   {
+    const int vext = P.perm[v];
+    const float h2m = P.h2_over_m[v];
     float* const scr = rb;   // [k][32][4] scratch
     for (int c = 0; c < kact; ++c) {
       float sx = 0.f, sy = 0.f, sz = 0.f;
@@ -321,22 +370,29 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       if (lane == 0) { float* q = scr + (c * 32 + warp) * 4; q[0] = sx; q[1] = sy; q[2] = sz; }
     }
     __syncthreads();
-    for (int c = 0; c < kact; ++c) {
-      const float* q = scr + (c * 32 + lane) * 4;
-      float cx = lane < nwarps ? q[0] : 0.f, cy = lane < nwarps ? q[1] : 0.f, cz = lane < nwarps ? q[2] : 0.f;
-      cx = warp_sum(cx); cy = warp_sum(cy); cz = warp_sum(cz);
-      const float invn = 1.0f / (float)n;
-      cx *= invn; cy *= invn; cz *= invn;
-      if (isv) {
-        const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
-        const float x0 = P.pos[g], x1 = P.pos[g + 1], x2 = P.pos[g + 2];
-        const float sx = (x0 - cx) + fmaf(h, P.vel[g], h2m * P.fext[g]);
-        const float sy = (x1 - cy) + fmaf(h, P.vel[g + 1], h2m * P.fext[g + 1]);
-        const float sz = (x2 - cz) + fmaf(h, P.vel[g + 2], h2m * P.fext[g + 2]);
-        s[(3 * c) * NP + v] = sx; s[(3 * c + 1) * NP + v] = sy; s[(3 * c + 2) * NP + v] = sz;
-        reinterpret_cast<float4*>(z4b)[c * NP + v] = make_float4(sx, sy, sz, 0.f);
+    float sreg[16], zero16[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { sreg[i] = 0.f; zero16[i] = 0.f; }
+#pragma unroll
+    for (int c = 0; c < kMaxCellsPerCta; ++c) {
+      if (c < kact) {
+        const float* q = scr + (c * 32 + lane) * 4;
+        float cx = lane < nwarps ? q[0] : 0.f, cy = lane < nwarps ? q[1] : 0.f, cz = lane < nwarps ? q[2] : 0.f;
+        cx = warp_sum(cx); cy = warp_sum(cy); cz = warp_sum(cz);
+        const float invn = 1.0f / (float)n;
+        cx *= invn; cy *= invn; cz *= invn;
+        if (isv) {
+          const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
+          const float sx = (P.pos[g] - cx) + fmaf(h, P.vel[g], h2m * P.fext[g]);
+          const float sy = (P.pos[g + 1] - cy) + fmaf(h, P.vel[g + 1], h2m * P.fext[g + 1]);
+          const float sz = (P.pos[g + 2] - cz) + fmaf(h, P.vel[g + 2], h2m * P.fext[g + 2]);
+          sreg[3 * c] = sx; sreg[3 * c + 1] = sy; sreg[3 * c + 2] = sz;
+          reinterpret_cast<float4*>(z4b)[c * NP + v] = make_float4(sx, sy, sz, 0.f);
+        }
       }
     }
+    tmem_st16(ta, sreg);
+    tmem_st16(ta + 16, zero16);
     __syncthreads();
   }
 
@@ -345,11 +401,13 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const float vol_dlen = kVolDTol * cbrtf(P.V0);
   const float vol_dtol2 = (float)n * vol_dlen * vol_dlen;
   const bool use_vol = P.w_volume > 0.0f;
+  const float4* const ec_t = ecs + (is_e ? tid : 0);
+  float4* const out_t = reinterpret_cast<float4*>(rbb) + (is_e ? tid : 0);
   for (int it = 0; it < P.n_iters; ++it) {
     // local step.  Pipeline over the CTA's cells, two barriers per cell:
     //   [elements(c) -> out] | [vertices(c): gather out, grad V, partial sums] | [elements(c+1);
     //   finish(c): volume multiplier, right-hand side] | ...
-    if (is_e) element_residual(er, z4b, P, reinterpret_cast<float4*>(rbb) + 4 * tid);
+    if (is_e) element_residual(ec_t, E, z4b, P, out_t);
     __syncthreads();
     for (int c = 0; c < kact; ++c) {
       const unsigned char* zc = z4b + c * cellz;
@@ -363,10 +421,13 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
             ev = ev + o;
           }
         }
-        for (int i = kRegList; i < icnt; ++i) ev = ev + lds3(rbb, inc_tail[i]);
+        if (icnt > kRegList) {
+          const uint16_t* inc_tail = P.inc_off + P.inc_ptr[v];
+          for (int i = kRegList; i < icnt; ++i) ev = ev + lds3(rbb, inc_tail[i]);
+        }
         if (use_vol) {
           zv = lds3(zc, v * 16);
-          g = ring_gradient(zc, zv, rcnt, roff, ring_tail);
+          g = ring_gradient(zc, zv, rcnt, roff, P, v);
           S1 = dot(zv, g);
           S2 = dot(g, g);
         }
@@ -377,11 +438,10 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       }
       __syncthreads();   // out consumed, partial sums complete
 
-      if (c + 1 < kact && is_e)
-        element_residual(er, z4b + (c + 1) * cellz, P, reinterpret_cast<float4*>(rbb) + 4 * tid);
+      if (c + 1 < kact && is_e) element_residual(ec_t, E, z4b + (c + 1) * cellz, P, out_t);
 
       // finish(c): D = lambda grad V(z + D), iterated (D <- ((g.D - C)/(g.g)) g,
-      // V = 1/3 sum_v z_v . g_v for the closed surface); stops early by kVolTol
+      // V = 1/3 sum_v z_v . g_v for the closed surface)
       F3 D = {0.f, 0.f, 0.f};
       if (use_vol) {
         float4 p4 = lane < nwarps ? red[c * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -409,7 +469,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           float S3 = 0.f;
           S1 = 0.f; S2 = 0.f;
           if (isv) {
-            g = ring_gradient(zc, zz, rcnt, roff, ring_tail);
+            g = ring_gradient(zc, zz, rcnt, roff, P, v);
             S1 = dot(zz, g); S2 = dot(g, g); S3 = dot(g, D);
           }
           S1 = warp_sum(S1); S2 = warp_sum(S2); S3 = warp_sum(S3);
@@ -428,14 +488,15 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         if (moved && isv) reinterpret_cast<float4*>(z4b + c * cellz)[v] = make_float4(zv.x, zv.y, zv.z, 0.f);
       }
       if (isv) {
-        // right-hand side of the global step, r = e - (m/h^2) d with e including w_vol D
+        // right-hand side of the global step, r = e - (m/h^2) d with e including w_vol D; the
+        // -(m/h^2) d part was left in place by the previous update pass
         const int m = 3 * c;
-        const float r0 = fmaf(P.w_volume, D.x, fmaf(-mh2, d[m * NP + v], ev.x));
-        const float r1 = fmaf(P.w_volume, D.y, fmaf(-mh2, d[(m + 1) * NP + v], ev.y));
-        const float r2 = fmaf(P.w_volume, D.z, fmaf(-mh2, d[(m + 2) * NP + v], ev.z));
-        ra[fbase + ((m) & 7) * 16 + ((m) >> 3)] = r0;
-        ra[fbase + ((m + 1) & 7) * 16 + ((m + 1) >> 3)] = r1;
-        ra[fbase + ((m + 2) & 7) * 16 + ((m + 2) >> 3)] = r2;
+        float* r0 = ra + fbase + ((m) & 7) * 16 + ((m) >> 3);
+        float* r1 = ra + fbase + ((m + 1) & 7) * 16 + ((m + 1) >> 3);
+        float* r2 = ra + fbase + ((m + 2) & 7) * 16 + ((m + 2) >> 3);
+        *r0 += fmaf(P.w_volume, D.x, ev.x);
+        *r1 += fmaf(P.w_volume, D.y, ev.y);
+        *r2 += fmaf(P.w_volume, D.z, ev.z);
       }
       __syncthreads();   // out(c+1) complete; z4 of cell c restored
     }
@@ -454,38 +515,38 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     }
     __syncthreads();
 
-    // global step: d += T r with T = A_sys^-1 in 8x8 blocks.  One warp per block of 8 output
-    // vertices: mma m16n8k8, M = the 16 right-hand-side columns, N = 8 output vertices, K = 8 source
-    // vertices per operator block; A fragments (hi, lo) are one LDS.128 each, the operator block
-    // comes straight from L2 and is split in registers (the tensor core ignores the low 13 bits).
-    {
-      const int g8 = lane >> 2, t4 = lane & 3;
-      const float4* const Ahi = reinterpret_cast<const float4*>(ra) + lane;
-      const float4* const Alo = reinterpret_cast<const float4*>(rb) + lane;
-      float* const z4f = reinterpret_cast<float*>(z4b);
-      // rows of the accumulator this lane owns: m = g8 and g8 + 8 (row 15 is the padding column)
-      const int m0 = g8, m1 = g8 + 8;
-      const int zo0 = ((m0 / 3) * NP) * 4 + (m0 % 3), zo1 = ((m1 / 3) * NP) * 4 + (m1 % 3);
-      for (int ib = warp; ib < nvb; ib += nwarps) {
-        float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    // global step: delta d = T r with T = A_sys^-1 in 8x8 blocks.  One warp per block of 8 output
+    // vertices (up to 4 blocks per warp): mma m16n8k8, M = the 16 right-hand-side columns, N = 8
+    // output vertices, K = 8 source vertices per operator block; A fragments (hi, lo) are one
+    // LDS.128 each, the operator block comes straight from L2 and is split in registers (the
+    // tensor core ignores the low 13 mantissa bits).
+    const int g8 = lane >> 2, t4 = lane & 3;
+    float acc[4][4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.f;
+      const int ib = warp + j * nwarps;
+      if (ib < nvb) {
         const int b0 = P.blk_ptr[ib], b1 = P.blk_ptr[ib + 1];
         if (MODE == 2) {
+          const float4* const Ahi = reinterpret_cast<const float4*>(ra) + lane;
+          const float4* const Alo = reinterpret_cast<const float4*>(rb) + lane;
           const float2* tv = reinterpret_cast<const float2*>(P.blk_val) + (size_t)b0 * 32 + lane;
           for (int bb = b0; bb < b1; bb += 32) {
             const int nb = min(32, b1 - bb);          // multiple of 4 (rows are padded)
             const int colv = lane < nb ? (int)P.blk_col[bb + lane] * 32 : 0;
             float2 cur[4], nxt[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) cur[u] = __ldg(tv + u * 32);
-            for (int j = 0; j < nb; j += 4) {
+            for (int u = 0; u < 4; ++u) { cur[u] = __ldg(tv + u * 32); nxt[u] = cur[u]; }
+            for (int jj = 0; jj < nb; jj += 4) {
               tv += 128;
-              if (j + 4 < nb) {
+              if (jj + 4 < nb) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u) nxt[u] = __ldg(tv + u * 32);
               }
 #pragma unroll
               for (int u = 0; u < 4; ++u) {
-                const int col = __shfl_sync(0xffffffffu, colv, j + u);
+                const int col = __shfl_sync(0xffffffffu, colv, jj + u);
                 const float4 ah = Ahi[col], al = Alo[col];
                 const uint32_t ahi[4] = {__float_as_uint(ah.x), __float_as_uint(ah.y),
                                          __float_as_uint(ah.z), __float_as_uint(ah.w)};
@@ -496,9 +557,9 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
                 const uint32_t bhi[2] = {bx, by};
                 const uint32_t blo[2] = {__float_as_uint(cur[u].x - __uint_as_float(bx)),
                                          __float_as_uint(cur[u].y - __uint_as_float(by))};
-                mma_tf32(acc, alo, bhi);
-                mma_tf32(acc, ahi, blo);
-                mma_tf32(acc, ahi, bhi);
+                mma_tf32(acc[j], alo, bhi);
+                mma_tf32(acc[j], ahi, blo);
+                mma_tf32(acc[j], ahi, bhi);
               }
 #pragma unroll
               for (int u = 0; u < 4; ++u) cur[u] = nxt[u];
@@ -519,49 +580,74 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
               // B(kk, i) sits at 2*((i<<2) | (kk&3)) + (kk>>2)
               const float bq0 = __ldg(tb + 2 * (((2 * t4) << 2) | (kk & 3)) + (kk >> 2));
               const float bq1 = __ldg(tb + 2 * (((2 * t4 + 1) << 2) | (kk & 3)) + (kk >> 2));
-              acc[0] = fmaf(a0, bq0, acc[0]); acc[1] = fmaf(a0, bq1, acc[1]);
-              acc[2] = fmaf(a1, bq0, acc[2]); acc[3] = fmaf(a1, bq1, acc[3]);
+              acc[j][0] = fmaf(a0, bq0, acc[j][0]); acc[j][1] = fmaf(a0, bq1, acc[j][1]);
+              acc[j][2] = fmaf(a1, bq0, acc[j][2]); acc[j][3] = fmaf(a1, bq1, acc[j][3]);
             }
           }
         }
-        // epilogue: d += acc, z = s + d for the lane's two rows and two adjacent output vertices
-        const int i0 = ib * 8 + 2 * t4;
-        if (m0 < 3 * P.k) {
-          float2* dp = reinterpret_cast<float2*>(d + m0 * NP + i0);
-          const float2 sv = *reinterpret_cast<const float2*>(s + m0 * NP + i0);
-          float2 dv = *dp;
-          dv.x += acc[0]; dv.y += acc[1];
-          *dp = dv;
-          z4f[zo0 + i0 * 4] = sv.x + dv.x;
-          z4f[zo0 + i0 * 4 + 4] = sv.y + dv.y;
-        }
-        if (m1 < 3 * P.k) {
-          float2* dp = reinterpret_cast<float2*>(d + m1 * NP + i0);
-          const float2 sv = *reinterpret_cast<const float2*>(s + m1 * NP + i0);
-          float2 dv = *dp;
-          dv.x += acc[2]; dv.y += acc[3];
-          *dp = dv;
-          z4f[zo1 + i0 * 4] = sv.x + dv.x;
-          z4f[zo1 + i0 * 4 + 4] = sv.y + dv.y;
-        }
       }
+    }
+    __syncthreads();   // every warp is done reading the right-hand sides
+
+    // hand the increments to the vertex owners: dd[m][NP] over the dead lo buffer
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int ib = warp + j * nwarps;
+      if (ib < nvb) {
+        const int i0 = ib * 8 + 2 * t4;
+        *reinterpret_cast<float2*>(rb + g8 * NP + i0) = make_float2(acc[j][0], acc[j][1]);
+        if (g8 < 7) *reinterpret_cast<float2*>(rb + (g8 + 8) * NP + i0) = make_float2(acc[j][2], acc[j][3]);
+      }
+    }
+    __syncthreads();
+
+    // owner update: d += delta d, z = s + d, and -(m/h^2) d as the start of the next rhs
+    {
+      float sv[16], dv[16];
+      tmem_ld16(ta, sv);
+      tmem_ld16(ta + 16, dv);
+#pragma unroll
+      for (int m = 0; m < 15; ++m) dv[m] += rb[m * NP + v];
+      if (isvp) {
+#pragma unroll
+        for (int c = 0; c < kMaxCellsPerCta; ++c)
+          if (c < P.k)
+            reinterpret_cast<float4*>(z4b)[c * NP + v] =
+                make_float4(sv[3 * c] + dv[3 * c], sv[3 * c + 1] + dv[3 * c + 1], sv[3 * c + 2] + dv[3 * c + 2], 0.f);
+#pragma unroll
+        for (int m = 0; m < 15; ++m) ra[fbase + (m & 7) * 16 + (m >> 3)] = -mh2 * dv[m];
+      }
+      tmem_st16(ta + 16, dv);
     }
     __syncthreads();
   }
 
   // ---- epilogue: x_n+1 = x_n + (u0 + d), v_n+1 = (u0 + d)/h
-  if (isv) {
-    const float invh = 1.0f / h;
-    for (int c = 0; c < kact; ++c) {
-      const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
+  {
+    float dv[16];
+    tmem_ld16(ta + 16, dv);
+    if (isv) {
+      const int vext = P.perm[v];
+      const float h2m = P.h2_over_m[v];
+      const float invh = 1.0f / h;
 #pragma unroll
-      for (int q = 0; q < 3; ++q) {
-        const float inc = fmaf(h, P.vel[g + q], h2m * P.fext[g + q]) + d[(3 * c + q) * NP + v];
-        P.pos[g + q] += inc;
-        P.vel[g + q] = inc * invh;
+      for (int c = 0; c < kMaxCellsPerCta; ++c) {
+        if (c < kact) {
+          const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            const float inc = fmaf(h, P.vel[g + q], h2m * P.fext[g + q]) + dv[3 * c + q];
+            P.pos[g + q] += inc;
+            P.vel[g + q] = inc * invh;
+          }
+        }
       }
     }
   }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0)
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base_s), "r"(tmem_cols) : "memory");
 }
 
 }  // namespace

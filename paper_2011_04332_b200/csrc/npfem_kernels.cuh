@@ -20,8 +20,7 @@ struct DevParams {
   float h, w_volume, V0, Vmin, Vmax;       // Vmin/Vmax = v_min*V0, v_max*V0
   float s_min, s_max, a_min, a_max;
   const uint16_t* perm;                    // [NP] internal -> caller vertex (padding: 0)
-  const uint32_t* elem_ids;                // [4][E] packed byte offsets 16*id: (a,b) (c,d) (f1,f2) (f3,f4)
-  const float* elem_f;                     // [kElemFloats][E] structure of arrays
+  const float4* elem_c;                    // [kElemGroups][E] element constants (npfem_api.cu)
   const float* h2_over_m;                  // [NP]
   const float* m_over_h2;                  // [NP]
   const uint16_t* inc_ptr;                 // [n+1]

@@ -575,7 +575,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     ec.f[30] = diamond ? 1.0f : 0.5f;
     const int nslots = diamond ? 4 : 3;
     for (int s = 0; s < nslots; ++s)
-      inc[P->iperm[idv[s]]].push_back((uint16_t)((e * 4 + s) * 16));
+      inc[P->iperm[idv[s]]].push_back((uint16_t)((s * E + e) * 16));
   }
   P->inc_ptr.assign(n + 1, 0);
   P->inc_off.clear();
