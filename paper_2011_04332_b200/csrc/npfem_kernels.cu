@@ -312,9 +312,9 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const int kact = min(P.k, P.n_cells - cell0);
   const int cellz = NP * 16;                      // bytes of one cell's z4
 
-  // ---- tensor memory: 32 columns (s: 0..14, d: 16..30) per group of 4 warps
-  uint32_t tmem_cols = 32;
-  while (tmem_cols < 32u * ((nwarps + 3) >> 2)) tmem_cols <<= 1;
+  // ---- tensor memory: 64 columns per group of 4 warps (s: 0..14, d: 16..30, u0: 32..46, x_n: 48..62)
+  uint32_t tmem_cols = 64;
+  while (tmem_cols < 64u * ((nwarps + 3) >> 2)) tmem_cols <<= 1;
   if (warp == 0) {
     const uint32_t sa = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(sa), "r"(tmem_cols) : "memory");
@@ -353,39 +353,50 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const uint32_t ta = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 32);
+  const uint32_t ta = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 64);
 
-  // ---- prologue: load state, centroid, local coordinates, inertial prediction
+  // ---- prologue: stage each cell's pos / vel / fext rows through shared memory with coalesced
+  //      loads, hand every vertex to its owner thread, centroid, local coordinates, prediction
+  const int vext3 = 3 * (int)P.perm[v];
   {
-    const int vext = P.perm[v];
     const float h2m = P.h2_over_m[v];
-    float* const scr = rb;   // [k][32][4] scratch
-    for (int c = 0; c < kact; ++c) {
-      float sx = 0.f, sy = 0.f, sz = 0.f;
-      if (isv) {
-        const float* px = P.pos + (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
-        sx = px[0]; sy = px[1]; sz = px[2];
-      }
-      sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
-      if (lane == 0) { float* q = scr + (c * 32 + warp) * 4; q[0] = sx; q[1] = sy; q[2] = sz; }
-    }
-    __syncthreads();
-    float sreg[16], zero16[16];
+    float* const st = rb;                    // [3][3n] staging (the element buffer is idle)
+    const int n3 = 3 * n;
+    float xr[16], ur[16], sreg[16], zero16[16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) { sreg[i] = 0.f; zero16[i] = 0.f; }
+    for (int i = 0; i < 16; ++i) { xr[i] = 0.f; ur[i] = 0.f; sreg[i] = 0.f; zero16[i] = 0.f; }
 #pragma unroll
     for (int c = 0; c < kMaxCellsPerCta; ++c) {
       if (c < kact) {
-        const float* q = scr + (c * 32 + lane) * 4;
-        float cx = lane < nwarps ? q[0] : 0.f, cy = lane < nwarps ? q[1] : 0.f, cz = lane < nwarps ? q[2] : 0.f;
-        cx = warp_sum(cx); cy = warp_sum(cy); cz = warp_sum(cz);
-        const float invn = 1.0f / (float)n;
-        cx *= invn; cy *= invn; cz *= invn;
+        const size_t g = (size_t)(cell0 + c) * P.cell_stride;
+        for (int i = tid; i < n3; i += blockDim.x) {
+          st[i] = P.pos[g + i]; st[n3 + i] = P.vel[g + i]; st[2 * n3 + i] = P.fext[g + i];
+        }
+        __syncthreads();
+        float sx = 0.f, sy = 0.f, sz = 0.f;
         if (isv) {
-          const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
-          const float sx = (P.pos[g] - cx) + fmaf(h, P.vel[g], h2m * P.fext[g]);
-          const float sy = (P.pos[g + 1] - cy) + fmaf(h, P.vel[g + 1], h2m * P.fext[g + 1]);
-          const float sz = (P.pos[g + 2] - cz) + fmaf(h, P.vel[g + 2], h2m * P.fext[g + 2]);
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            xr[3 * c + q] = st[vext3 + q];
+            ur[3 * c + q] = fmaf(h, st[n3 + vext3 + q], h2m * st[2 * n3 + vext3 + q]);
+          }
+          sx = xr[3 * c]; sy = xr[3 * c + 1]; sz = xr[3 * c + 2];
+        }
+        sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
+        if (lane == 0) red[c * 32 + warp] = make_float4(sx, sy, sz, 0.f);
+        __syncthreads();   // staging is reused by the next cell; partial sums complete
+      }
+    }
+#pragma unroll
+    for (int c = 0; c < kMaxCellsPerCta; ++c) {
+      if (c < kact) {
+        const float4 p4 = lane < nwarps ? red[c * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float invn = 1.0f / (float)n;
+        const float cx = warp_sum(p4.x) * invn, cy = warp_sum(p4.y) * invn, cz = warp_sum(p4.z) * invn;
+        if (isv) {
+          const float sx = (xr[3 * c] - cx) + ur[3 * c];
+          const float sy = (xr[3 * c + 1] - cy) + ur[3 * c + 1];
+          const float sz = (xr[3 * c + 2] - cz) + ur[3 * c + 2];
           sreg[3 * c] = sx; sreg[3 * c + 1] = sy; sreg[3 * c + 2] = sz;
           reinterpret_cast<float4*>(z4b)[c * NP + v] = make_float4(sx, sy, sz, 0.f);
         }
@@ -393,6 +404,8 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     }
     tmem_st16(ta, sreg);
     tmem_st16(ta + 16, zero16);
+    tmem_st16(ta + 32, ur);
+    tmem_st16(ta + 48, xr);
     __syncthreads();
   }
 
@@ -502,16 +515,17 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     }
 
     // split the right-hand sides into tf32 high and low parts (hi in place, lo over the dead
-    // element buffer).  Round-to-nearest on the 13 dropped mantissa bits; lo = x - hi is exact.
-    if (isvp) {
-#pragma unroll
-      for (int m = 0; m < kRhs; ++m) {
-        const int idx = fbase + (m & 7) * 16 + (m >> 3);
-        const float x = ra[idx];
-        const float hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
-        ra[idx] = hi;
-        rb[idx] = x - hi;
-      }
+    // element buffer), one float4 per thread and trip: conflict-free.  Round-to-nearest on the 13
+    // dropped mantissa bits; lo = x - hi is exact.
+    for (int q = tid; q < NP * 4; q += blockDim.x) {
+      const float4 x = reinterpret_cast<const float4*>(ra)[q];
+      float4 hi;
+      hi.x = __uint_as_float((__float_as_uint(x.x) + 0x1000u) & 0xffffe000u);
+      hi.y = __uint_as_float((__float_as_uint(x.y) + 0x1000u) & 0xffffe000u);
+      hi.z = __uint_as_float((__float_as_uint(x.z) + 0x1000u) & 0xffffe000u);
+      hi.w = __uint_as_float((__float_as_uint(x.w) + 0x1000u) & 0xffffe000u);
+      reinterpret_cast<float4*>(ra)[q] = hi;
+      reinterpret_cast<float4*>(rb)[q] = make_float4(x.x - hi.x, x.y - hi.y, x.z - hi.z, x.w - hi.w);
     }
     __syncthreads();
 
@@ -529,40 +543,52 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       if (ib < nvb) {
         const int b0 = P.blk_ptr[ib], b1 = P.blk_ptr[ib + 1];
         if (MODE == 2) {
-          const float4* const Ahi = reinterpret_cast<const float4*>(ra) + lane;
-          const float4* const Alo = reinterpret_cast<const float4*>(rb) + lane;
+          const unsigned char* const Ahi = reinterpret_cast<const unsigned char*>(ra) + lane * 16;
+          const int lo_off = P.L.rb - P.L.ra;
           const float2* tv = reinterpret_cast<const float2*>(P.blk_val) + (size_t)b0 * 32 + lane;
+          // four operator blocks: A fragments by LDS.128 at the block's byte offset, 3xTF32 mma
+          auto mma4 = [&](const float2 (&tb)[4], int colv, int jbase) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const int col = __shfl_sync(0xffffffffu, colv, jbase + u);
+              const float4 ah = *reinterpret_cast<const float4*>(Ahi + col);
+              const float4 al = *reinterpret_cast<const float4*>(Ahi + col + lo_off);
+              const uint32_t ahi[4] = {__float_as_uint(ah.x), __float_as_uint(ah.y),
+                                       __float_as_uint(ah.z), __float_as_uint(ah.w)};
+              const uint32_t alo[4] = {__float_as_uint(al.x), __float_as_uint(al.y),
+                                       __float_as_uint(al.z), __float_as_uint(al.w)};
+              const uint32_t bx = __float_as_uint(tb[u].x) & 0xffffe000u;
+              const uint32_t by = __float_as_uint(tb[u].y) & 0xffffe000u;
+              const uint32_t bhi[2] = {bx, by};
+              const uint32_t blo[2] = {__float_as_uint(tb[u].x - __uint_as_float(bx)),
+                                       __float_as_uint(tb[u].y - __uint_as_float(by))};
+              mma_tf32(acc[j], alo, bhi);
+              mma_tf32(acc[j], ahi, blo);
+              mma_tf32(acc[j], ahi, bhi);
+            }
+          };
           for (int bb = b0; bb < b1; bb += 32) {
             const int nb = min(32, b1 - bb);          // multiple of 4 (rows are padded)
-            const int colv = lane < nb ? (int)P.blk_col[bb + lane] * 32 : 0;
-            float2 cur[4], nxt[4];
+            const int colv = lane < nb ? (int)P.blk_col[bb + lane] * 512 : 0;   // byte offset of block jb
+            float2 t0[4], t1[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) { cur[u] = __ldg(tv + u * 32); nxt[u] = cur[u]; }
-            for (int jj = 0; jj < nb; jj += 4) {
-              tv += 128;
+            for (int u = 0; u < 4; ++u) { t0[u] = __ldg(tv + u * 32); t1[u] = t0[u]; }
+            for (int jj = 0; jj < nb; jj += 8) {     // software pipeline, two stages of 4 blocks
               if (jj + 4 < nb) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) nxt[u] = __ldg(tv + u * 32);
+                for (int u = 0; u < 4; ++u) t1[u] = __ldg(tv + 128 + u * 32);
               }
+              mma4(t0, colv, jj);
+              tv += 256;
+              if (jj + 4 < nb) {
+                if (jj + 8 < nb) {
 #pragma unroll
-              for (int u = 0; u < 4; ++u) {
-                const int col = __shfl_sync(0xffffffffu, colv, jj + u);
-                const float4 ah = Ahi[col], al = Alo[col];
-                const uint32_t ahi[4] = {__float_as_uint(ah.x), __float_as_uint(ah.y),
-                                         __float_as_uint(ah.z), __float_as_uint(ah.w)};
-                const uint32_t alo[4] = {__float_as_uint(al.x), __float_as_uint(al.y),
-                                         __float_as_uint(al.z), __float_as_uint(al.w)};
-                const uint32_t bx = __float_as_uint(cur[u].x) & 0xffffe000u;
-                const uint32_t by = __float_as_uint(cur[u].y) & 0xffffe000u;
-                const uint32_t bhi[2] = {bx, by};
-                const uint32_t blo[2] = {__float_as_uint(cur[u].x - __uint_as_float(bx)),
-                                         __float_as_uint(cur[u].y - __uint_as_float(by))};
-                mma_tf32(acc[j], alo, bhi);
-                mma_tf32(acc[j], ahi, blo);
-                mma_tf32(acc[j], ahi, bhi);
+                  for (int u = 0; u < 4; ++u) t0[u] = __ldg(tv + u * 32);
+                }
+                mma4(t1, colv, jj + 4);
+              } else {
+                tv -= 128;
               }
-#pragma unroll
-              for (int u = 0; u < 4; ++u) cur[u] = nxt[u];
             }
           }
         } else {
@@ -622,25 +648,31 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     __syncthreads();
   }
 
-  // ---- epilogue: x_n+1 = x_n + (u0 + d), v_n+1 = (u0 + d)/h
+  // ---- epilogue: x_n+1 = x_n + (u0 + d), v_n+1 = (u0 + d)/h, staged in caller order through
+  //      shared memory so that the stores to pos / vel are coalesced
   {
-    float dv[16];
+    float dv[16], ur[16], xr[16];
     tmem_ld16(ta + 16, dv);
-    if (isv) {
-      const int vext = P.perm[v];
-      const float h2m = P.h2_over_m[v];
-      const float invh = 1.0f / h;
+    tmem_ld16(ta + 32, ur);
+    tmem_ld16(ta + 48, xr);
+    float* const st = rb;                    // [2][3n]
+    const int n3 = 3 * n;
+    const float invh = 1.0f / h;
 #pragma unroll
-      for (int c = 0; c < kMaxCellsPerCta; ++c) {
-        if (c < kact) {
-          const size_t g = (size_t)(cell0 + c) * P.cell_stride + 3 * vext;
+    for (int c = 0; c < kMaxCellsPerCta; ++c) {
+      if (c < kact) {
+        if (isv) {
 #pragma unroll
           for (int q = 0; q < 3; ++q) {
-            const float inc = fmaf(h, P.vel[g + q], h2m * P.fext[g + q]) + dv[3 * c + q];
-            P.pos[g + q] += inc;
-            P.vel[g + q] = inc * invh;
+            const float inc = ur[3 * c + q] + dv[3 * c + q];
+            st[vext3 + q] = xr[3 * c + q] + inc;
+            st[n3 + vext3 + q] = inc * invh;
           }
         }
+        __syncthreads();
+        const size_t g = (size_t)(cell0 + c) * P.cell_stride;
+        for (int i = tid; i < n3; i += blockDim.x) { P.pos[g + i] = st[i]; P.vel[g + i] = st[n3 + i]; }
+        __syncthreads();
       }
     }
   }
