@@ -201,10 +201,26 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
     for (int hgi = 0; hgi < 5; ++hgi)
       for (int q = 0; q < 4; ++q) W(4 + hgi, q) = fbits(ec.f[10 + 4 * hgi + q]);
   }
+  // vertex-role constants, two uint4 per (padded) vertex, fetched by the owner thread just before
+  // its vertex phase: [0] = first 6 element-slot byte offsets (u16 pairs), icnt | rcnt << 8;
+  // [1] = first 6 ring byte offsets (u16 pairs), bits of m/h^2.  Longer lists continue in
+  // inc_off / ring_off.
+  std::vector<uint32_t> vrole((size_t)NP * 8, 0u);
+  for (int i = 0; i < n; ++i) {
+    const int i0 = P.inc_ptr[i], icnt = P.inc_ptr[i + 1] - i0;
+    const int r0 = P.ring_ptr[i], rcnt = P.ring_ptr[i + 1] - r0;
+    uint32_t* w = &vrole[(size_t)i * 8];
+    for (int q = 0; q < kRegList; ++q) {
+      if (q < icnt) w[q >> 1] |= (uint32_t)P.inc_off[i0 + q] << (16 * (q & 1));
+      if (q < rcnt) w[4 + (q >> 1)] |= (uint32_t)P.ring_off[r0 + q] << (16 * (q & 1));
+    }
+    w[3] = (uint32_t)(icnt > 255 ? 255 : icnt) | (uint32_t)(rcnt > 255 ? 255 : rcnt) << 8;
+    w[7] = fbits(P.m_over_h2[i]);
+  }
   struct Sec { const void* src; size_t bytes; size_t off; };
   Sec secs[] = {
       {perm16.data(), perm16.size() * 2, 0},          {elem_c.data(), elem_c.size() * 4, 0},
-      {nullptr, 0, 0},                                {h2m.data(), h2m.size() * 4, 0},
+      {vrole.data(), vrole.size() * 4, 0},            {h2m.data(), h2m.size() * 4, 0},
       {mh2.data(), mh2.size() * 4, 0},                {P.inc_ptr.data(), P.inc_ptr.size() * 2, 0},
       {P.inc_off.data(), P.inc_off.size() * 2, 0},    {P.ring_ptr.data(), P.ring_ptr.size() * 2, 0},
       {P.ring_off.data(), P.ring_off.size() * 2, 0},  {P.blk_ptr.data(), P.blk_ptr.size() * 4, 0},
@@ -229,6 +245,7 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.a_min = (float)P.mat.a_min; D.a_max = (float)P.mat.a_max;
   D.perm = reinterpret_cast<const uint16_t*>(base + secs[0].off);
   D.elem_c = reinterpret_cast<const float4*>(base + secs[1].off);
+  D.vrole = reinterpret_cast<const uint4*>(base + secs[2].off);
   D.h2_over_m = reinterpret_cast<const float*>(base + secs[3].off);
   D.m_over_h2 = reinterpret_cast<const float*>(base + secs[4].off);
   D.inc_ptr = reinterpret_cast<const uint16_t*>(base + secs[5].off);

@@ -178,6 +178,13 @@ __device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], 
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
 }
 
+// Operator blocks stream from L2 once per use: keep them out of L1, which holds the register spills.
+__device__ __forceinline__ float2 ldg_stream(const float2* p) {
+  float2 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  return v;
+}
+
 // ---- tensor memory as per-thread scratch: thread (warp w, lane l) owns TMEM lane 32*(w%4) + l;
 //      a 32x32b.x16 access moves 16 consecutive columns of that lane to / from 16 registers.
 __device__ __forceinline__ void tmem_st16(uint32_t a, const float (&v)[16]) {
@@ -267,8 +274,9 @@ __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, 
 // grad V at a vertex = 1/6 sum over its fan of (r_i - z) x (r_i+1 - z); the first kRegList ring
 // offsets come from registers, longer fans continue from the global list.
 __device__ __forceinline__ F3 ring_gradient(const unsigned char* zc, F3 zv, int rcnt,
-                                            const uint32_t (&roff)[kRegList / 2],
+                                            uint32_t roff0, uint32_t roff1, uint32_t roff2,
                                             const DevParams& P, int v) {
+  const uint32_t roff[kRegList / 2] = {roff0, roff1, roff2};
   const F3 e0 = lds3(zc, roff[0] & 0xffffu) - zv;
   F3 ep = e0, g = {0.f, 0.f, 0.f};
 #pragma unroll
@@ -324,21 +332,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   // ---- per-thread constants of the vertex role
   const bool is_e = tid < E, isv = tid < n, isvp = tid < NP;
   const int v = isvp ? tid : 0;
-  const float mh2 = P.m_over_h2[v];
   const float h = P.h;
-  int icnt = 0, rcnt = 0;
-  uint32_t ioff[kRegList / 2] = {0, 0, 0}, roff[kRegList / 2] = {0, 0, 0};
-  if (isv) {
-    const int i0 = P.inc_ptr[v], r0 = P.ring_ptr[v];
-    icnt = P.inc_ptr[v + 1] - i0;
-    rcnt = P.ring_ptr[v + 1] - r0;
-#pragma unroll
-    for (int i = 0; i < kRegList; ++i) {
-      const uint32_t io = i < icnt ? P.inc_off[i0 + i] : 0u, ro = i < rcnt ? P.ring_off[r0 + i] : 0u;
-      ioff[i >> 1] |= io << (16 * (i & 1));
-      roff[i >> 1] |= ro << (16 * (i & 1));
-    }
-  }
   // float index of (vertex v, rhs column 0) in the A-fragment layout:
   //   block jb = v/8 holds 32 lanes x float4; lane = (m&7)*4 + (v&3), component = 2*((v&7)>>2) + (m>>3)
   const int fbase = ((v >> 3) * 32 + (v & 3)) * 4 + 2 * ((v & 7) >> 2);
@@ -421,12 +415,18 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     //   [elements(c) -> out] | [vertices(c): gather out, grad V, partial sums] | [elements(c+1);
     //   finish(c): volume multiplier, right-hand side] | ...
     if (is_e) element_residual(ec_t, E, z4b, P, out_t);
+    // vertex-role constants (npfem_api.cu: vrole) are fetched just before they are needed instead
+    // of living in registers across the element pass: x = inc offsets 0..5 (3 words) + counts,
+    // y = ring offsets 0..5 (3 words) + m/h^2
+    uint4 vr0 = P.vrole[2 * v], vr1 = P.vrole[2 * v + 1];
     __syncthreads();
     for (int c = 0; c < kact; ++c) {
       const unsigned char* zc = z4b + c * cellz;
+      const int icnt = vr0.w & 0xff, rcnt = (vr0.w >> 8) & 0xff;
       F3 ev = {0.f, 0.f, 0.f}, g = {0.f, 0.f, 0.f}, zv = {0.f, 0.f, 0.f};
       float S1 = 0.f, S2 = 0.f;
       if (isv) {
+        const uint32_t ioff[kRegList / 2] = {vr0.x, vr0.y, vr0.z};
 #pragma unroll
         for (int i = 0; i < kRegList; ++i) {
           if (i < icnt) {
@@ -440,7 +440,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         }
         if (use_vol) {
           zv = lds3(zc, v * 16);
-          g = ring_gradient(zc, zv, rcnt, roff, P, v);
+          g = ring_gradient(zc, zv, rcnt, vr1.x, vr1.y, vr1.z, P, v);
           S1 = dot(zv, g);
           S2 = dot(g, g);
         }
@@ -450,8 +450,6 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         if (lane == 0) red[c * 32 + warp] = make_float4(S1, S2, 0.f, 0.f);
       }
       __syncthreads();   // out consumed, partial sums complete
-
-      if (c + 1 < kact && is_e) element_residual(ec_t, E, z4b + (c + 1) * cellz, P, out_t);
 
       // finish(c): D = lambda grad V(z + D), iterated (D <- ((g.D - C)/(g.g)) g,
       // V = 1/3 sum_v z_v . g_v for the closed surface)
@@ -482,7 +480,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           float S3 = 0.f;
           S1 = 0.f; S2 = 0.f;
           if (isv) {
-            g = ring_gradient(zc, zz, rcnt, roff, P, v);
+            g = ring_gradient(zc, zz, rcnt, vr1.x, vr1.y, vr1.z, P, v);
             S1 = dot(zz, g); S2 = dot(g, g); S3 = dot(g, D);
           }
           S1 = warp_sum(S1); S2 = warp_sum(S2); S3 = warp_sum(S3);
@@ -510,6 +508,10 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         *r0 += fmaf(P.w_volume, D.x, ev.x);
         *r1 += fmaf(P.w_volume, D.y, ev.y);
         *r2 += fmaf(P.w_volume, D.z, ev.z);
+      }
+      if (c + 1 < kact) {
+        if (is_e) element_residual(ec_t, E, z4b + (c + 1) * cellz, P, out_t);
+        vr0 = P.vrole[2 * v]; vr1 = P.vrole[2 * v + 1];
       }
       __syncthreads();   // out(c+1) complete; z4 of cell c restored
     }
@@ -547,6 +549,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           const int lo_off = P.L.rb - P.L.ra;
           const float2* tv = reinterpret_cast<const float2*>(P.blk_val) + (size_t)b0 * 32 + lane;
           // four operator blocks: A fragments by LDS.128 at the block's byte offset, 3xTF32 mma
+          float accx[4] = {0.f, 0.f, 0.f, 0.f};
           auto mma4 = [&](const float2 (&tb)[4], int colv, int jbase) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
@@ -562,8 +565,8 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
               const uint32_t bhi[2] = {bx, by};
               const uint32_t blo[2] = {__float_as_uint(tb[u].x - __uint_as_float(bx)),
                                        __float_as_uint(tb[u].y - __uint_as_float(by))};
-              mma_tf32(acc[j], alo, bhi);
-              mma_tf32(acc[j], ahi, blo);
+              mma_tf32(accx, alo, bhi);      // the two correction terms and the main term go to
+              mma_tf32(accx, ahi, blo);      // separate accumulators: two dependency chains
               mma_tf32(acc[j], ahi, bhi);
             }
           };
@@ -572,18 +575,18 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
             const int colv = lane < nb ? (int)P.blk_col[bb + lane] * 512 : 0;   // byte offset of block jb
             float2 t0[4], t1[4];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) { t0[u] = __ldg(tv + u * 32); t1[u] = t0[u]; }
+            for (int u = 0; u < 4; ++u) { t0[u] = ldg_stream(tv + u * 32); t1[u] = t0[u]; }
             for (int jj = 0; jj < nb; jj += 8) {     // software pipeline, two stages of 4 blocks
               if (jj + 4 < nb) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) t1[u] = __ldg(tv + 128 + u * 32);
+                for (int u = 0; u < 4; ++u) t1[u] = ldg_stream(tv + 128 + u * 32);
               }
               mma4(t0, colv, jj);
               tv += 256;
               if (jj + 4 < nb) {
                 if (jj + 8 < nb) {
 #pragma unroll
-                  for (int u = 0; u < 4; ++u) t0[u] = __ldg(tv + u * 32);
+                  for (int u = 0; u < 4; ++u) t0[u] = ldg_stream(tv + u * 32);
                 }
                 mma4(t1, colv, jj + 4);
               } else {
@@ -591,6 +594,8 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
               }
             }
           }
+#pragma unroll
+          for (int q = 0; q < 4; ++q) acc[j][q] += accx[q];
         } else {
           // fp32 comparison path: the same sums with plain FMAs, operands re-read per term
           for (int b = b0; b < b1; ++b) {
@@ -630,6 +635,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     // owner update: d += delta d, z = s + d, and -(m/h^2) d as the start of the next rhs
     {
       float sv[16], dv[16];
+      const float nmh2 = -__uint_as_float(P.vrole[2 * v + 1].w);
       tmem_ld16(ta, sv);
       tmem_ld16(ta + 16, dv);
 #pragma unroll
@@ -641,7 +647,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
             reinterpret_cast<float4*>(z4b)[c * NP + v] =
                 make_float4(sv[3 * c] + dv[3 * c], sv[3 * c + 1] + dv[3 * c + 1], sv[3 * c + 2] + dv[3 * c + 2], 0.f);
 #pragma unroll
-        for (int m = 0; m < 15; ++m) ra[fbase + (m & 7) * 16 + (m >> 3)] = -mh2 * dv[m];
+        for (int m = 0; m < 15; ++m) ra[fbase + (m & 7) * 16 + (m >> 3)] = nmh2 * dv[m];
       }
       tmem_st16(ta + 16, dv);
     }

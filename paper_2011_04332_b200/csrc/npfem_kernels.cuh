@@ -23,6 +23,7 @@ struct DevParams {
   const float4* elem_c;                    // [kElemGroups][E] element constants (npfem_api.cu)
   const float* h2_over_m;                  // [NP]
   const float* m_over_h2;                  // [NP]
+  const uint4* vrole;                      // [NP][2] vertex-role constants (npfem_api.cu)
   const uint16_t* inc_ptr;                 // [n+1]
   const uint16_t* inc_off;                 // byte offsets into the element result buffer
   const uint16_t* ring_ptr;                // [n+1]
