@@ -131,8 +131,7 @@ __device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, flo
   const F3 F0 = i00 * e1;
   const F3 F1 = fma3(i01, e1, i11 * e2);
   const float C11 = dot(F0, F0), C12 = dot(F0, F1), C22 = dot(F1, F1);
-  const F3 Nn = cross(F0, F1);
-  const float J = fsqrt(dot(Nn, Nn));                         // sigma1 * sigma2
+  const float J = fsqrt(fmaxf(fmaf(C11, C22, -C12 * C12), 0.0f));   // sigma1 * sigma2 = sqrt(det F^T F)
   const float tau = fsqrt(C11 + C22 + 2.0f * J);              // sigma1 + sigma2
   const float dC = C11 - C22;
   const float Delta = fsqrt(fmaf(dC, dC, 4.0f * C12 * C12));  // sigma1^2 - sigma2^2
@@ -219,16 +218,8 @@ __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, 
   const F3 eab = zb - za, eac = zc3 - za, ebc = zc3 - zb, ead = zd - za, ebd = zd - zb;
   const F3 eba = {-eab.x, -eab.y, -eab.z};
 
-  // ---- membranes: t1 = (a,b,c) from a; t2 = (b,a,d) from b
-  const float4 m1 = ec[E], m2 = ec[2 * E], m3 = ec[3 * E];
-  F3 t1b, t1c, t2a, t2d;
-  membrane(eab, eac, m1.x, m1.y, m1.z, m1.w, m3.x, P, t1b, t1c);
-  membrane(eba, ebd, m2.x, m2.y, m2.z, m2.w, m3.y, P, t2a, t2d);
-  F3 fa = t2a - (t1b + t1c);
-  F3 fb = t1b - (t2a + t2d);
-  F3 fc = t1c;
-  F3 fd = t2d;
-
+  F3 fa = {0.f, 0.f, 0.f}, fb = fa, fc = fa, fd = fa;
+  const float4 m3 = ec[3 * E];
   // ---- shared hinge (a,b | c ; d): once in full for a diamond, the element's half for a single
   {
     const float4 hk = ec[4 * E];
@@ -264,6 +255,18 @@ __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, 
     const F3 edb = {-ebd.x, -ebd.y, -ebd.z}, eda = {-ead.x, -ead.y, -ead.z};
     const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, edb, eda, zf - zd);
     fd = fma3(0.5f * hk.x, kv, fd); fb = fma3(0.5f * hk.y, kv, fb); fa = fma3(hk.z, kv, fa);
+  }
+  // ---- membranes, last (the hinge pass is over, few values are live): t1 = (a,b,c) from a;
+  //      t2 = (b,a,d) from b
+  {
+    const float4 m1 = ec[E], m2 = ec[2 * E];
+    F3 t1b, t1c, t2a, t2d;
+    membrane(eab, eac, m1.x, m1.y, m1.z, m1.w, m3.x, P, t1b, t1c);
+    membrane(eba, ebd, m2.x, m2.y, m2.z, m2.w, m3.y, P, t2a, t2d);
+    fa = fa + (t2a - (t1b + t1c));
+    fb = fb + (t1b - (t2a + t2d));
+    fc = fc + t1c;
+    fd = fd + t2d;
   }
   out4[0] = make_float4(fa.x, fa.y, fa.z, 0.0f);
   out4[E] = make_float4(fb.x, fb.y, fb.z, 0.0f);
@@ -412,19 +415,39 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   float4* const out_t = reinterpret_cast<float4*>(rbb) + (is_e ? tid : 0);
   for (int it = 0; it < P.n_iters; ++it) {
     // local step.  Pipeline over the CTA's cells, two barriers per cell:
-    //   [elements(c) -> out] | [vertices(c): gather out, grad V, partial sums] | [elements(c+1);
-    //   finish(c): volume multiplier, right-hand side] | ...
-    if (is_e) element_residual(ec_t, E, z4b, P, out_t);
-    // vertex-role constants (npfem_api.cu: vrole) are fetched just before they are needed instead
-    // of living in registers across the element pass: x = inc offsets 0..5 (3 words) + counts,
-    // y = ring offsets 0..5 (3 words) + m/h^2
-    uint4 vr0 = P.vrole[2 * v], vr1 = P.vrole[2 * v + 1];
+    //   [elements(c) -> out; volume gradient(c), partial sums] | [vertices(c): gather out, volume
+    //   multiplier, right-hand side] | [elements(c+1); ...] | ...
+    // The volume gradient only reads z, so every warp runs its share right after its elements:
+    // warps that finish the element pass early keep working instead of waiting at the barrier.
+    // Vertex-role constants (npfem_api.cu: vrole) are fetched just before they are needed instead
+    // of living in registers across the element pass: [0] = element-slot offsets 0..5 (3 words) +
+    // counts, [1] = ring offsets 0..5 (3 words) + m/h^2.
+    F3 g = {0.f, 0.f, 0.f}, zv = {0.f, 0.f, 0.f};
+    uint4 vr0;
+    auto elements_and_gradient = [&](int cc) {
+      const unsigned char* zcc = z4b + cc * cellz;
+      if (is_e) element_residual(ec_t, E, zcc, P, out_t);
+      vr0 = P.vrole[2 * v];
+      if (use_vol) {
+        float S1 = 0.f, S2 = 0.f;
+        if (isv) {
+          const uint4 vr1 = P.vrole[2 * v + 1];
+          zv = lds3(zcc, v * 16);
+          g = ring_gradient(zcc, zv, (vr0.w >> 8) & 0xff, vr1.x, vr1.y, vr1.z, P, v);
+          S1 = dot(zv, g);
+          S2 = dot(g, g);
+        }
+        S1 = warp_sum(S1); S2 = warp_sum(S2);
+        if (lane == 0) red[cc * 32 + warp] = make_float4(S1, S2, 0.f, 0.f);
+      }
+    };
+    elements_and_gradient(0);
     __syncthreads();
     for (int c = 0; c < kact; ++c) {
       const unsigned char* zc = z4b + c * cellz;
       const int icnt = vr0.w & 0xff, rcnt = (vr0.w >> 8) & 0xff;
-      F3 ev = {0.f, 0.f, 0.f}, g = {0.f, 0.f, 0.f}, zv = {0.f, 0.f, 0.f};
-      float S1 = 0.f, S2 = 0.f;
+      F3 ev = {0.f, 0.f, 0.f};
+      float S1, S2;
       if (isv) {
         const uint32_t ioff[kRegList / 2] = {vr0.x, vr0.y, vr0.z};
 #pragma unroll
@@ -438,18 +461,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           const uint16_t* inc_tail = P.inc_off + P.inc_ptr[v];
           for (int i = kRegList; i < icnt; ++i) ev = ev + lds3(rbb, inc_tail[i]);
         }
-        if (use_vol) {
-          zv = lds3(zc, v * 16);
-          g = ring_gradient(zc, zv, rcnt, vr1.x, vr1.y, vr1.z, P, v);
-          S1 = dot(zv, g);
-          S2 = dot(g, g);
-        }
       }
-      if (use_vol) {
-        S1 = warp_sum(S1); S2 = warp_sum(S2);
-        if (lane == 0) red[c * 32 + warp] = make_float4(S1, S2, 0.f, 0.f);
-      }
-      __syncthreads();   // out consumed, partial sums complete
 
       // finish(c): D = lambda grad V(z + D), iterated (D <- ((g.D - C)/(g.g)) g,
       // V = 1/3 sum_v z_v . g_v for the closed surface)
@@ -480,6 +492,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           float S3 = 0.f;
           S1 = 0.f; S2 = 0.f;
           if (isv) {
+            const uint4 vr1 = P.vrole[2 * v + 1];
             g = ring_gradient(zc, zz, rcnt, vr1.x, vr1.y, vr1.z, P, v);
             S1 = dot(zz, g); S2 = dot(g, g); S3 = dot(g, D);
           }
@@ -509,11 +522,11 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         *r1 += fmaf(P.w_volume, D.y, ev.y);
         *r2 += fmaf(P.w_volume, D.z, ev.z);
       }
+      __syncthreads();   // out consumed; right-hand side of cell c complete; z4 of cell c restored
       if (c + 1 < kact) {
-        if (is_e) element_residual(ec_t, E, z4b + (c + 1) * cellz, P, out_t);
-        vr0 = P.vrole[2 * v]; vr1 = P.vrole[2 * v + 1];
+        elements_and_gradient(c + 1);
+        __syncthreads();   // out(c+1) and the partial sums of cell c+1 complete
       }
-      __syncthreads();   // out(c+1) complete; z4 of cell c restored
     }
 
     // split the right-hand sides into tf32 high and low parts (hi in place, lo over the dead
