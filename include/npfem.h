@@ -134,6 +134,9 @@ typedef struct {
   int op_nnz;          /* entries of A_sys^-1 kept by the drop rule (before blocking) */
   int global_mode;     /* 1 = SIMT, 2 = 3xTF32 */
   int volume_inner_iters;
+  int n_op_blocks_tf32x1; /* of n_op_blocks, blocks applied as ONE TF32 product: their share of   */
+                          /* every row's l1 mass is <= 2^-15, so the product error stays below   */
+                          /* fp32 rounding of the row sum; all other blocks use 3xTF32            */
   double rest_volume, total_mass, inv_drop_tol;
 } npfem_info;
 int npfem_get_info(npfem_handle h, npfem_info* out);

@@ -53,6 +53,7 @@ void fill_info(const Plan& P, int cell_stride, npfem_info* o) {
   o->smem_bytes = P.smem_bytes;
   o->n_vblocks = P.nvb;
   o->n_op_blocks = P.n_op_blocks;
+  o->n_op_blocks_tf32x1 = P.n_op_blocks_x1;
   o->op_nnz = P.op_nnz;
   o->global_mode = P.global_mode;
   o->volume_inner_iters = P.opt.volume_inner_iters;
@@ -129,7 +130,7 @@ int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems) {
       double* D = static_cast<double*>(dst);
       std::memset(D, 0, elems * sizeof(double));
       for (int ib = 0; ib < P.nvb; ++ib)
-        for (int b = P.blk_ptr[ib]; b < P.blk_ptr[ib + 1]; ++b) {
+        for (int b = P.blk_ptr[3 * ib]; b < P.blk_ptr[3 * ib + 2]; ++b) {
           const int jb = P.blk_col[b];
           for (int l = 0; l < 32; ++l)
             for (int r = 0; r < 2; ++r) {

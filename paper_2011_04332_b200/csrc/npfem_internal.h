@@ -68,10 +68,11 @@ struct Plan {
   std::vector<uint16_t> ring_ptr;    // [n+1] CSR over the cyclically ordered ring neighbours
   std::vector<uint16_t> ring_off;    // byte offset (16 * internal id) of the neighbour in z4
   int nvb = 0;                       // number of 8-vertex blocks
-  std::vector<int32_t> blk_ptr;      // [nvb+1] operator blocks per OUTPUT block (rows padded to x4)
+  std::vector<int32_t> blk_ptr;      // [nvb][3] per OUTPUT block row: first 3xTF32 block, first 1xTF32 block, end
   std::vector<uint16_t> blk_col;     // [n_blocks_padded] source block index
   std::vector<float> blk_val;        // [n_blocks_padded][64] in mma B-fragment order
   int n_op_blocks = 0;               // kept blocks (without the zero padding blocks)
+  int n_op_blocks_x1 = 0;            // of those, blocks applied as one TF32 product
   int op_nnz = 0;
 
   // launch configuration decided at create time

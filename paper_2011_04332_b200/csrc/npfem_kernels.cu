@@ -302,6 +302,69 @@ __device__ __forceinline__ F3 ring_gradient(const unsigned char* zc, F3 zv, int 
   return (1.0f / 6.0f) * g;
 }
 
+// One run of operator blocks [b0, b1) of an output block row (a multiple of 4 blocks), software-
+// pipelined in two stages of 4 blocks: the operator blocks stream from L2 (one float2 per lane
+// and block, mma B-fragment order), the A fragments come by LDS.128 from the right-hand sides
+// at the source block's byte offset.  FULL: 3xTF32 -- the block is split in registers (the
+// tensor core ignores the low 13 mantissa bits) and the two correction terms go to a second
+// accumulator (two dependency chains).  !FULL: blocks whose share of the row's l1 mass is below
+// 2^-15 (npfem_plan.cpp): a single TF32 product is then exact to fp32 rounding of the row sum.
+template <bool FULL>
+__device__ __forceinline__ void block_run(float (&acc)[4], float (&accx)[4], const float2* tv,
+                                          const uint16_t* __restrict__ blk_col, int b0, int b1,
+                                          const unsigned char* Ahi, int lo_off, int lane) {
+  tv += (size_t)b0 * 32;
+  auto mma4 = [&](const float2 (&tb)[4], int colv, int jbase) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int col = __shfl_sync(0xffffffffu, colv, jbase + u);
+      const float4 ah = *reinterpret_cast<const float4*>(Ahi + col);
+      const uint32_t ahi[4] = {__float_as_uint(ah.x), __float_as_uint(ah.y),
+                               __float_as_uint(ah.z), __float_as_uint(ah.w)};
+      if (FULL) {
+        const float4 al = *reinterpret_cast<const float4*>(Ahi + col + lo_off);
+        const uint32_t alo[4] = {__float_as_uint(al.x), __float_as_uint(al.y),
+                                 __float_as_uint(al.z), __float_as_uint(al.w)};
+        const uint32_t bx = __float_as_uint(tb[u].x) & 0xffffe000u;
+        const uint32_t by = __float_as_uint(tb[u].y) & 0xffffe000u;
+        const uint32_t bhi[2] = {bx, by};
+        const uint32_t blo[2] = {__float_as_uint(tb[u].x - __uint_as_float(bx)),
+                                 __float_as_uint(tb[u].y - __uint_as_float(by))};
+        mma_tf32(accx, alo, bhi);
+        mma_tf32(accx, ahi, blo);
+        mma_tf32(acc, ahi, bhi);
+      } else {
+        const uint32_t braw[2] = {__float_as_uint(tb[u].x), __float_as_uint(tb[u].y)};
+        mma_tf32(accx, ahi, braw);
+      }
+    }
+  };
+  for (int bb = b0; bb < b1; bb += 32) {
+    const int nb = min(32, b1 - bb);          // multiple of 4 (runs are padded)
+    const int colv = lane < nb ? (int)blk_col[bb + lane] * 512 : 0;   // byte offset of block jb
+    float2 t0[4], t1[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { t0[u] = ldg_stream(tv + u * 32); t1[u] = t0[u]; }
+    for (int jj = 0; jj < nb; jj += 8) {
+      if (jj + 4 < nb) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) t1[u] = ldg_stream(tv + 128 + u * 32);
+      }
+      mma4(t0, colv, jj);
+      tv += 256;
+      if (jj + 4 < nb) {
+        if (jj + 8 < nb) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) t0[u] = ldg_stream(tv + u * 32);
+        }
+        mma4(t1, colv, jj + 4);
+      } else {
+        tv -= 128;
+      }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // The fused step kernel.  MODE 1: global step with fp32 FMAs (comparison path); MODE 2: 3xTF32
 // mma.sync on the block-sparse inverse.
@@ -544,11 +607,9 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     }
     __syncthreads();
 
-    // global step: delta d = T r with T = A_sys^-1 in 8x8 blocks.  One warp per block of 8 output
-    // vertices (up to 4 blocks per warp): mma m16n8k8, M = the 16 right-hand-side columns, N = 8
-    // output vertices, K = 8 source vertices per operator block; A fragments (hi, lo) are one
-    // LDS.128 each, the operator block comes straight from L2 and is split in registers (the
-    // tensor core ignores the low 13 mantissa bits).
+    // global step: delta d = T r with T = A_sys^-1 in 8x8 blocks.  One warp per block row of 8
+    // output vertices (up to 4 rows per warp): mma m16n8k8, M = the 16 right-hand-side columns,
+    // N = 8 output vertices, K = 8 source vertices per operator block (block_run above).
     const int g8 = lane >> 2, t4 = lane & 3;
     float acc[4][4];
 #pragma unroll
@@ -556,57 +617,13 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.f;
       const int ib = warp + j * nwarps;
       if (ib < nvb) {
-        const int b0 = P.blk_ptr[ib], b1 = P.blk_ptr[ib + 1];
+        const int b0 = P.blk_ptr[3 * ib], bm = P.blk_ptr[3 * ib + 1], b1 = P.blk_ptr[3 * ib + 2];
         if (MODE == 2) {
           const unsigned char* const Ahi = reinterpret_cast<const unsigned char*>(ra) + lane * 16;
-          const int lo_off = P.L.rb - P.L.ra;
-          const float2* tv = reinterpret_cast<const float2*>(P.blk_val) + (size_t)b0 * 32 + lane;
-          // four operator blocks: A fragments by LDS.128 at the block's byte offset, 3xTF32 mma
+          const float2* const tv = reinterpret_cast<const float2*>(P.blk_val) + lane;
           float accx[4] = {0.f, 0.f, 0.f, 0.f};
-          auto mma4 = [&](const float2 (&tb)[4], int colv, int jbase) {
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-              const int col = __shfl_sync(0xffffffffu, colv, jbase + u);
-              const float4 ah = *reinterpret_cast<const float4*>(Ahi + col);
-              const float4 al = *reinterpret_cast<const float4*>(Ahi + col + lo_off);
-              const uint32_t ahi[4] = {__float_as_uint(ah.x), __float_as_uint(ah.y),
-                                       __float_as_uint(ah.z), __float_as_uint(ah.w)};
-              const uint32_t alo[4] = {__float_as_uint(al.x), __float_as_uint(al.y),
-                                       __float_as_uint(al.z), __float_as_uint(al.w)};
-              const uint32_t bx = __float_as_uint(tb[u].x) & 0xffffe000u;
-              const uint32_t by = __float_as_uint(tb[u].y) & 0xffffe000u;
-              const uint32_t bhi[2] = {bx, by};
-              const uint32_t blo[2] = {__float_as_uint(tb[u].x - __uint_as_float(bx)),
-                                       __float_as_uint(tb[u].y - __uint_as_float(by))};
-              mma_tf32(accx, alo, bhi);      // the two correction terms and the main term go to
-              mma_tf32(accx, ahi, blo);      // separate accumulators: two dependency chains
-              mma_tf32(acc[j], ahi, bhi);
-            }
-          };
-          for (int bb = b0; bb < b1; bb += 32) {
-            const int nb = min(32, b1 - bb);          // multiple of 4 (rows are padded)
-            const int colv = lane < nb ? (int)P.blk_col[bb + lane] * 512 : 0;   // byte offset of block jb
-            float2 t0[4], t1[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) { t0[u] = ldg_stream(tv + u * 32); t1[u] = t0[u]; }
-            for (int jj = 0; jj < nb; jj += 8) {     // software pipeline, two stages of 4 blocks
-              if (jj + 4 < nb) {
-#pragma unroll
-                for (int u = 0; u < 4; ++u) t1[u] = ldg_stream(tv + 128 + u * 32);
-              }
-              mma4(t0, colv, jj);
-              tv += 256;
-              if (jj + 4 < nb) {
-                if (jj + 8 < nb) {
-#pragma unroll
-                  for (int u = 0; u < 4; ++u) t0[u] = ldg_stream(tv + u * 32);
-                }
-                mma4(t1, colv, jj + 4);
-              } else {
-                tv -= 128;
-              }
-            }
-          }
+          block_run<true>(acc[j], accx, tv, P.blk_col, b0, bm, Ahi, P.L.rb - P.L.ra, lane);
+          block_run<false>(acc[j], accx, tv, P.blk_col, bm, b1, Ahi, 0, lane);
 #pragma unroll
           for (int q = 0; q < 4; ++q) acc[j][q] += accx[q];
         } else {

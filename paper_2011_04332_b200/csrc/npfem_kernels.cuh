@@ -28,7 +28,7 @@ struct DevParams {
   const uint16_t* inc_off;                 // byte offsets into the element result buffer
   const uint16_t* ring_ptr;                // [n+1]
   const uint16_t* ring_off;                // byte offsets into one cell's z4
-  const int* blk_ptr;                      // [nvb+1]
+  const int* blk_ptr;                      // [nvb][3]: first 3xTF32 block, first 1xTF32 block, end
   const uint16_t* blk_col;                 // [n_blocks_padded]
   const float* blk_val;                    // [n_blocks_padded][64]
   float* pos;

@@ -10,6 +10,7 @@
 // No CUDA here: this file is plain C++ so that the CPU tests can exercise it through
 // npfem_plan_create / npfem_plan_query.
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstring>
 #include <deque>
@@ -349,35 +350,82 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
         bmask[(size_t)(P->iperm[i] / 8) * nvb + P->iperm[j] / 8] = 1;
       }
   P->op_nnz = nnz;
-  // rows of blocks are padded with all-zero blocks to a multiple of 4 so that the kernel's
-  // unrolled, software-pipelined block loop needs no tail handling
-  P->blk_ptr.assign(nvb + 1, 0);
+  // Per output block row: first the blocks applied with 3xTF32, then the blocks whose entries are
+  // so small that ONE TF32 product is exact to fp32 rounding of the row sum: a TF32 product of
+  // truncated operands errs by < 2^-9 relative, so blocks are moved to the second run, smallest
+  // first, while their l1 mass stays <= 2^-15 of the l1 norm of EVERY row of the block row
+  // (product error <= 2^-24 ||row||_1 |r|_max, the size of one fp32 rounding).  Each run is padded
+  // with all-zero blocks to a multiple of 4 for the kernel's unrolled, software-pipelined loop.
+  P->blk_ptr.assign(3 * (size_t)nvb, 0);
   P->blk_col.clear();
   P->blk_val.clear();
   P->n_op_blocks = 0;
-  for (int ib = 0; ib < nvb; ++ib) {
-    int row_blocks = 0;
-    for (int jb = 0; jb < nvb; ++jb) {
-      if (!bmask[(size_t)ib * nvb + jb]) continue;
+  P->n_op_blocks_x1 = 0;
+  {
+    const double tier_tol = std::ldexp(1.0, -15);
+    auto Tint = [&](int i, int j) {   // operator entry in internal numbering, 0 outside
+      return (i < n && j < n) ? Tinv[(size_t)P->perm[i] * n + P->perm[j]] : 0.0;
+    };
+    auto emit = [&](int ib, int jb, bool zero) {
       P->blk_col.push_back((uint16_t)jb);
       size_t base = P->blk_val.size();
       P->blk_val.resize(base + 64, 0.0f);
+      if (zero) return;
       for (int l = 0; l < 32; ++l)
         for (int r = 0; r < 2; ++r) {
           int j = jb * 8 + (l & 3) + 4 * r;   // source vertex (k index of the mma B fragment)
           int i = ib * 8 + (l >> 2);          // output vertex (n index)
-          if (i < n && j < n)
-            P->blk_val[base + 2 * l + r] = (float)Tinv[(size_t)P->perm[i] * n + P->perm[j]];
+          P->blk_val[base + 2 * l + r] = (float)Tint(i, j);
         }
-      ++row_blocks;
-      ++P->n_op_blocks;
+    };
+    for (int ib = 0; ib < nvb; ++ib) {
+      std::vector<int> cols;
+      for (int jb = 0; jb < nvb; ++jb)
+        if (bmask[(size_t)ib * nvb + jb]) cols.push_back(jb);
+      // l1 mass of each kept block per row of the block row, and the rows' l1 norms over kept blocks
+      std::vector<std::array<double, 8>> mass(cols.size());
+      std::array<double, 8> rowl1{};
+      for (size_t q = 0; q < cols.size(); ++q)
+        for (int r = 0; r < 8; ++r) {
+          double m = 0.0;
+          for (int cc = 0; cc < 8; ++cc) m += std::fabs(Tint(ib * 8 + r, cols[q] * 8 + cc));
+          mass[q][r] = m;
+          rowl1[r] += m;
+        }
+      std::vector<int> order(cols.size());
+      std::iota(order.begin(), order.end(), 0);
+      auto bmax = [&](int q) { return *std::max_element(mass[q].begin(), mass[q].end()); };
+      std::sort(order.begin(), order.end(), [&](int p, int q) {
+        double mp = bmax(p), mq = bmax(q);
+        return mp != mq ? mp < mq : p < q;
+      });
+      std::vector<uint8_t> single(cols.size(), 0);
+      std::array<double, 8> cum{};
+      for (int q : order) {
+        bool ok = cols[q] != ib;   // the diagonal block always stays in the 3xTF32 run
+        for (int r = 0; r < 8 && ok; ++r)
+          if (rowl1[r] > 0.0 && cum[r] + mass[q][r] > tier_tol * rowl1[r]) ok = false;
+        if (!ok) break;
+        for (int r = 0; r < 8; ++r) cum[r] += mass[q][r];
+        single[q] = 1;
+      }
+      for (int pass = 0; pass < 2; ++pass) {
+        P->blk_ptr[3 * (size_t)ib + pass] = (int32_t)P->blk_col.size();
+        int run_blocks = 0;
+        for (size_t q = 0; q < cols.size(); ++q) {
+          if ((int)single[q] != pass) continue;
+          emit(ib, cols[q], false);
+          ++run_blocks;
+          ++P->n_op_blocks;
+          P->n_op_blocks_x1 += pass;
+        }
+        while (run_blocks % 4) {
+          emit(ib, ib, true);
+          ++run_blocks;
+        }
+      }
+      P->blk_ptr[3 * (size_t)ib + 2] = (int32_t)P->blk_col.size();
     }
-    while (row_blocks % 4) {
-      P->blk_col.push_back((uint16_t)ib);
-      P->blk_val.resize(P->blk_val.size() + 64, 0.0f);
-      ++row_blocks;
-    }
-    P->blk_ptr[ib + 1] = (int32_t)P->blk_col.size();
   }
 
   // ---- per-vertex constants (internal numbering)
