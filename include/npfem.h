@@ -66,6 +66,8 @@ typedef struct {
   int volume_inner_iters; /* iterations of the volume projection per local step (>= 1); default 2  */
   int cells_per_cta;      /* 1..5 cells share one CTA and every fetched operator block; 0 = auto   */
   int global_mode;        /* 0 = auto, 1 = fp32 SIMT blocks, 2 = 3xTF32 tensor-core blocks          */
+  int pair_triangles;     /* local-step work items: 0 = auto / 1 = pairs of triangles across a shared */
+                          /* edge wherever the matching finds one, 2 = one triangle per item        */
 } npfem_options;
 
 /*
@@ -137,6 +139,8 @@ typedef struct {
   int n_op_blocks_tf32x1; /* of n_op_blocks, blocks applied as ONE TF32 product: their share of   */
                           /* every row's l1 mass is <= 2^-15, so the product error stays below   */
                           /* fp32 rounding of the row sum; all other blocks use 3xTF32            */
+  int n_elements;         /* threads' work items of the local step: pairs of triangles sharing an  */
+  int n_diamonds;         /* edge (n_diamonds of them) plus triangles left single by the matching  */
   double rest_volume, total_mass, inv_drop_tol;
 } npfem_info;
 int npfem_get_info(npfem_handle h, npfem_info* out);
@@ -162,6 +166,8 @@ int npfem_plan_info(npfem_plan p, npfem_info* out);
 #define NPFEM_Q_HINGE_WR 7    /* double [n_hinges][2]: (w_h, r_h)                                  */
 #define NPFEM_Q_TRI_DMINV 8   /* double [n_tris][3]: (i00, i01, i11) of D_m^-1                     */
 #define NPFEM_Q_TRI_AREA 9    /* double [n_tris]                                                   */
+#define NPFEM_Q_OPERATOR_X1 10 /* double [n_verts^2]: like NPFEM_Q_OPERATOR, only the blocks that are    */
+                              /* applied as one TF32 product (npfem_info.n_op_blocks_tf32x1)       */
 int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems);
 
 #ifdef __cplusplus

@@ -17,7 +17,8 @@ MATERIAL_FIELDS = ("cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min",
 
 QUERY = {"perm": (1, np.int32), "mass": (2, np.float64), "system": (3, np.float64),
          "operator": (4, np.float64), "hinge_verts": (5, np.int32), "hinge_K": (6, np.float64),
-         "hinge_wr": (7, np.float64), "tri_dminv": (8, np.float64), "tri_area": (9, np.float64)}
+         "hinge_wr": (7, np.float64), "tri_dminv": (8, np.float64), "tri_area": (9, np.float64),
+         "operator_x1": (10, np.float64)}
 
 ERROR_NAMES = {0: "NPFEM_OK", -1: "NPFEM_EINVAL", -2: "NPFEM_ENOMEM", -3: "NPFEM_ECUDA",
                -4: "NPFEM_ELIMIT"}
@@ -29,14 +30,14 @@ class Material(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("inv_drop_tol", C.c_double), ("volume_inner_iters", C.c_int),
-                ("cells_per_cta", C.c_int), ("global_mode", C.c_int)]
+                ("cells_per_cta", C.c_int), ("global_mode", C.c_int), ("pair_triangles", C.c_int)]
 
 
 class Info(C.Structure):
     _fields_ = [(f, C.c_int) for f in (
         "n_verts", "n_tris", "n_hinges", "cell_stride", "cells_per_cta", "threads_per_cta",
         "smem_bytes", "n_vblocks", "n_op_blocks", "op_nnz", "global_mode",
-        "volume_inner_iters", "n_op_blocks_tf32x1")] + [(f, C.c_double) for f in ("rest_volume", "total_mass",
+        "volume_inner_iters", "n_op_blocks_tf32x1", "n_elements", "n_diamonds")] + [(f, C.c_double) for f in ("rest_volume", "total_mass",
                                                             "inv_drop_tol")]
 
     def as_dict(self) -> dict:
@@ -102,9 +103,10 @@ def _material(mat: dict) -> Material:
     return Material(**{k: float(mat[k]) for k in MATERIAL_FIELDS})
 
 
-def _options(inv_drop_tol=None, volume_inner_iters=0, cells_per_cta=0, global_mode=0) -> Options:
+def _options(inv_drop_tol=None, volume_inner_iters=0, cells_per_cta=0, global_mode=0,
+             pair_triangles=0) -> Options:
     return Options(-1.0 if inv_drop_tol is None else float(inv_drop_tol), int(volume_inner_iters),
-                   int(cells_per_cta), int(global_mode))
+                   int(cells_per_cta), int(global_mode), int(pair_triangles))
 
 
 def _mesh_args(tris, rest_xyz):

@@ -54,6 +54,8 @@ void fill_info(const Plan& P, int cell_stride, npfem_info* o) {
   o->n_vblocks = P.nvb;
   o->n_op_blocks = P.n_op_blocks;
   o->n_op_blocks_tf32x1 = P.n_op_blocks_x1;
+  o->n_elements = P.E;
+  o->n_diamonds = P.n_diamonds;
   o->op_nnz = P.op_nnz;
   o->global_mode = P.global_mode;
   o->volume_inner_iters = P.opt.volume_inner_iters;
@@ -123,14 +125,15 @@ int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems) {
     case NPFEM_Q_HINGE_WR: return copy_out(P.hinge_wr.data(), 2 * (size_t)P.H, sizeof(double));
     case NPFEM_Q_TRI_DMINV: return copy_out(P.tri_dminv.data(), 3 * (size_t)P.T, sizeof(double));
     case NPFEM_Q_TRI_AREA: return copy_out(P.tri_area.data(), (size_t)P.T, sizeof(double));
-    case NPFEM_Q_OPERATOR: {
+    case NPFEM_Q_OPERATOR:
+    case NPFEM_Q_OPERATOR_X1: {
       const size_t elems = (size_t)n * n;
       if (!dst) return (int)elems;
       if ((size_t)dst_elems < elems) return set_err(NPFEM_EINVAL, "destination too small");
       double* D = static_cast<double*>(dst);
       std::memset(D, 0, elems * sizeof(double));
       for (int ib = 0; ib < P.nvb; ++ib)
-        for (int b = P.blk_ptr[3 * ib]; b < P.blk_ptr[3 * ib + 2]; ++b) {
+        for (int b = P.blk_ptr[3 * ib + (what == NPFEM_Q_OPERATOR_X1 ? 1 : 0)]; b < P.blk_ptr[3 * ib + 2]; ++b) {
           const int jb = P.blk_col[b];
           for (int l = 0; l < 32; ++l)
             for (int r = 0; r < 2; ++r) {

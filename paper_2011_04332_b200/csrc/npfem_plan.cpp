@@ -135,12 +135,14 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     o.volume_inner_iters = opts->volume_inner_iters;
     o.cells_per_cta = opts->cells_per_cta;
     o.global_mode = opts->global_mode;
+    o.pair_triangles = opts->pair_triangles;
   }
   if (o.volume_inner_iters <= 0) o.volume_inner_iters = 2;
   if (o.volume_inner_iters > 8) o.volume_inner_iters = 8;
   if (o.cells_per_cta < 0 || o.cells_per_cta > kMaxCellsPerCta)
     return fail(NPFEM_EINVAL, "cells_per_cta must be 0..5");
   if (o.global_mode < 0 || o.global_mode > 2) return fail(NPFEM_EINVAL, "global_mode must be 0..2");
+  if (o.pair_triangles < 0 || o.pair_triangles > 2) return fail(NPFEM_EINVAL, "pair_triangles must be 0..2");
   P->tris_ext.assign(tris, tris + 3 * T);
   auto Xv = [&](int v) { return V3{X[3 * v], X[3 * v + 1], X[3 * v + 2]}; };
 
@@ -513,6 +515,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
         mate[u] = -1;
       }
     }
+    if (o.pair_triangles == 2) std::fill(mate.begin(), mate.end(), -1);
     // sanity: mate must be an involution
     for (int t = 0; t < T; ++t)
       if (mate[t] >= 0 && (mate[t] == t || mate[mate[t]] != t)) {

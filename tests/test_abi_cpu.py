@@ -97,6 +97,34 @@ def test_operator_is_the_inverse_up_to_the_drop_rule(cell):
     assert dense.info()["n_op_blocks"] == dense.info()["n_vblocks"] ** 2
 
 
+def test_single_tf32_blocks_stay_below_fp32_rounding_of_the_row_sum(cell):
+    """Blocks applied as ONE TF32 product (error < 2^-9 per product of truncated operands) may hold
+    at most 2^-15 of any row's l1 mass, so their total error stays below 2^-24 ||row||_1 |r|_max."""
+    rest, tris, mat, plan, oc = cell
+    n = rest.shape[0]
+    info = plan.info()
+    op = plan.query("operator").reshape(n, n)
+    x1 = plan.query("operator_x1").reshape(n, n)
+    assert 0 <= info["n_op_blocks_tf32x1"] < info["n_op_blocks"]
+    assert np.array_equal(x1[x1 != 0], op[x1 != 0])                     # a subset of the operator
+    assert (np.diag(x1) == 0).all()                                     # never the diagonal blocks
+    share = np.abs(x1).sum(axis=1) / np.abs(op).sum(axis=1)
+    assert share.max() <= 2.0 ** -15 * (1 + 1e-6)
+    if n >= 600:                                                        # RBC-3: the tier is really used
+        assert info["n_op_blocks_tf32x1"] > info["n_op_blocks"] // 4
+
+
+def test_elements_pair_all_triangles_of_the_icospheres(cell):
+    """The local step works on elements = pairs of triangles across a shared edge (a matching of
+    the dual graph); on the icospheres the matching is perfect, so E = T/2 threads do the work."""
+    rest, tris, mat, plan, oc = cell
+    info = plan.info()
+    T = tris.shape[0]
+    assert 2 * info["n_diamonds"] + (info["n_elements"] - info["n_diamonds"]) == T
+    assert info["n_elements"] == T // 2 and info["n_diamonds"] == T // 2
+    assert info["threads_per_cta"] >= max(info["n_elements"], rest.shape[0])
+
+
 def test_increment_form_with_the_kept_operator_reproduces_oracle_iterates():
     """The algebra of the kernel, d <- d + T (f_int(s + d) - (m/h^2) d), evaluated in fp64 with
     the plan's (dropped, fp32-rounded) operator, against the oracle's absolute-form iterates."""

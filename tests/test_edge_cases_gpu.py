@@ -151,6 +151,53 @@ def test_shrunk_and_inflated_cells_exercise_volume_and_area_projection():
     _parity(g, forces * 3, 10, volume_inner_iters=8)
 
 
+def _split_triangles(rest, tris, which):
+    """1 -> 3 split of the chosen triangles (new vertex at the centroid): valence-3 vertices, and
+    every corner of a split triangle gains one neighbour."""
+    rest = [np.asarray(p, dtype=np.float64) for p in rest]
+    out = []
+    for ti, (a, b, c) in enumerate(tris.tolist()):
+        if ti in which:
+            m = len(rest)
+            rest.append((rest[a] + rest[b] + rest[c]) / 3.0)
+            out += [(a, b, m), (b, c, m), (c, a, m)]
+        else:
+            out.append((a, b, c))
+    return np.array(rest), np.array(out, dtype=np.int32)
+
+
+def test_irregular_mesh_with_valence_3_and_12_vertices():
+    """Vertex fans longer than the 6 entries a thread keeps in registers (a valence-12 vertex) and
+    valence-3 vertices: the overflow lists of the gather and of the volume gradient."""
+    rest, tris = W.rest_shape("rbc", 2)
+    rng = np.random.Generator(np.random.PCG64(11))
+    hub = 17
+    which = set(np.nonzero((tris == hub).any(axis=1))[0].tolist()) | set(
+        rng.choice(tris.shape[0], size=18, replace=False).tolist())
+    rest, tris = _split_triangles(rest, tris, which)
+    assert np.bincount(tris.ravel()).max() == 12 and np.bincount(tris.ravel()).min() == 3
+    mat = W.default_material(rest, tris)
+    rot, trans = W.random_rigid_placements(6, 100.0, 5.0, rng)
+    pos0 = W.place_cells(rest, rot, trans)
+    vel0 = (rng.standard_normal(pos0.shape) * 1e-4).astype(np.float32)
+    forces = [W.gaussian_forces(pos0.shape, 1e-3, 11, s) for s in range(3)]
+    _parity(_G(rest, tris, mat, pos0, vel0), forces, 8)
+
+
+def test_unpaired_triangles_one_element_per_triangle():
+    """pair_triangles = 2: every triangle is a single-triangle element (the shared hinge is then
+    evaluated half by each side, nothing is written for the fourth vertex)."""
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=6)
+    g = _G(rest, tris, mat, pos0, vel0)
+    h = NpfemHandle(tris, rest, mat, 0.1, pair_triangles=2)
+    assert h.info()["n_diamonds"] == 0 and h.info()["n_elements"] == tris.shape[0]
+    _parity(g, forces, 8, pair_triangles=2)
+    # and it is the same computation as the paired default up to fp32 summation order
+    a = list(gpu_trajectory(g, 0.1, forces, 8))[-1][0]
+    b = list(gpu_trajectory(g, 0.1, forces, 8, pair_triangles=2))[-1][0]
+    assert np.abs(a.astype(np.float64) - b).max() <= 4e-6
+
+
 def test_step_host_matches_device_step_bit_for_bit_and_is_deterministic():
     rest, tris, mat, pos0, vel0, forces = _small_workload(level=3, n_cells=23)
     n = rest.shape[0]
