@@ -62,6 +62,21 @@ def hbm_bytes_per_cell_step(n_verts: int) -> int:
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x FMA x max clock
 
 
+def measured_dram_traffic(n_verts: int, n_cells: int):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the step kernel,
+    from the committed `ncu --set full` capture: profiles/r1c_dram_traffic.csv holds the bytes per
+    cell measured there; a launch moves that times its cells.  None without a capture."""
+    path = os.path.join(ROOT, "profiles", "r1c_dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as fh:
+        rows = [ln.strip().split(",") for ln in fh if ln.strip() and not ln.startswith("#")]
+    rec = dict(zip(rows[0], rows[1]))
+    if int(rec["n_verts"]) != n_verts:
+        return None
+    return float(rec["dram_bytes_per_cell"]) * n_cells
+
+
 def load_peaks() -> dict:
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -313,7 +328,7 @@ def run_ours(args) -> None:
     achieved_tflops = f_alg / (launch_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS_NOMINAL,
                 "unit": "TFLOP/s", "frac": achieved_tflops / FP32_PEAK_TFLOPS_NOMINAL,
-                "traffic": None, "kernel": "npfem_step_kernel",
+                "traffic": measured_dram_traffic(n, n_cells), "kernel": "npfem_step_kernel",
                 "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
                 "algorithmic_flops_per_launch": f_alg, "launch_ms": launch_ms,
                 "hbm": {"achieved_gbs": b_alg / (launch_ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
@@ -336,7 +351,8 @@ def run_ours(args) -> None:
                        "n_cells_per_gpu": n_cells, "n_verts": n, "n_iters": n_iters,
                        "cells_per_cta": info["cells_per_cta"], "threads_per_cta": info["threads_per_cta"],
                        "smem_bytes": info["smem_bytes"], "global_mode": info["global_mode"],
-                       "op_blocks": info["n_op_blocks"],
+                       "op_blocks": info["n_op_blocks"], "op_blocks_tf32x1": info["n_op_blocks_tf32x1"],
+                       "elements_per_cell": info["n_elements"],
                        "l2": "inputs (2.3 GB per step) exceed L2; no flush needed"},
             "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "clocks": clocks,
             "state_finite": finite}
