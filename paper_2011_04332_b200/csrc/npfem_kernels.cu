@@ -20,7 +20,8 @@
 // per own vertex; thread v < n owns one VERTEX, gathers its element slots, evaluates grad V on
 // its ring and forms the right-hand side; the global step then multiplies all 16 right-hand-side
 // columns of the CTA by the block-sparse inverse on the tensor cores (3xTF32 split, fp32
-// accumulate).  s and d, private to the owner thread, live in tensor memory (TMEM).
+// accumulate).  s, d, the elastic residual and u0, private to the owner thread, live in tensor
+// memory (TMEM).
 #include <cstdint>
 
 #include "npfem_kernels.cuh"
@@ -35,9 +36,6 @@ __device__ __forceinline__ F3 operator+(F3 a, F3 b) { return {a.x + b.x, a.y + b
 __device__ __forceinline__ F3 operator-(F3 a, F3 b) { return {a.x - b.x, a.y - b.y, a.z - b.z}; }
 __device__ __forceinline__ F3 operator*(float s, F3 a) { return {s * a.x, s * a.y, s * a.z}; }
 __device__ __forceinline__ float dot(F3 a, F3 b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }
-__device__ __forceinline__ F3 cross(F3 a, F3 b) {
-  return {fmaf(a.y, b.z, -a.z * b.y), fmaf(a.z, b.x, -a.x * b.z), fmaf(a.x, b.y, -a.y * b.x)};
-}
 // acc + a x b
 __device__ __forceinline__ F3 cross_acc(F3 a, F3 b, F3 acc) {
   return {fmaf(a.y, b.z, fmaf(-a.z, b.y, acc.x)), fmaf(a.z, b.x, fmaf(-a.x, b.z, acc.y)),
@@ -204,6 +202,11 @@ __device__ __forceinline__ void tmem_st16(uint32_t a, const float (&v)[16]) {
       :: "r"(a), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]),
          "f"(v[8]), "f"(v[9]), "f"(v[10]), "f"(v[11]), "f"(v[12]), "f"(v[13]), "f"(v[14]), "f"(v[15])
       : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_st4(uint32_t a, float v0, float v1, float v2, float v3) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
+               :: "r"(a), "f"(v0), "f"(v1), "f"(v2), "f"(v3) : "memory");
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
@@ -387,7 +390,8 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   unsigned char* const z4b = smem_raw + P.L.z4;                        // [k][NP] float4 iterate z
   const float4* const ecs = reinterpret_cast<const float4*>(smem_raw + P.L.ec);   // element constants
   float* const ra = reinterpret_cast<float*>(smem_raw + P.L.ra);       // rhs, A-fragment order (fp32 / hi)
-  unsigned char* const rbb = smem_raw + P.L.rb;                        // element results / rhs lo / delta d
+  unsigned char* const rab = smem_raw + P.L.ra;                        // element results (odd cells) / rhs hi
+  unsigned char* const rbb = smem_raw + P.L.rb;                        // element results (even cells) / rhs lo / delta d
   float* const rb = reinterpret_cast<float*>(rbb);
   float4* const red = reinterpret_cast<float4*>(smem_raw + P.L.red);   // [5][32] partial sums
   __shared__ uint32_t tmem_base_s;
@@ -398,7 +402,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const int kact = min(P.k, P.n_cells - cell0);
   const int cellz = NP * 16;                      // bytes of one cell's z4
 
-  // ---- tensor memory: 64 columns per group of 4 warps (s: 0..14, d: 16..30, u0: 32..46, x_n: 48..62)
+  // ---- tensor memory: 64 columns per group of 4 warps (s: 0..14, d: 16..30, rhs: 32..47, u0: 48..62)
   uint32_t tmem_cols = 64;
   while (tmem_cols < 64u * ((nwarps + 3) >> 2)) tmem_cols <<= 1;
   if (warp == 0) {
@@ -476,8 +480,8 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     }
     tmem_st16(ta, sreg);
     tmem_st16(ta + 16, zero16);
-    tmem_st16(ta + 32, ur);
-    tmem_st16(ta + 48, xr);
+    tmem_st16(ta + 32, zero16);
+    tmem_st16(ta + 48, ur);
     __syncthreads();
   }
 
@@ -487,7 +491,6 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const float vol_dtol2 = (float)n * vol_dlen * vol_dlen;
   const bool use_vol = P.w_volume > 0.0f;
   const float4* const ec_t = ecs + (is_e ? tid : 0);
-  float4* const out_t = reinterpret_cast<float4*>(rbb) + (is_e ? tid : 0);
   for (int it = 0; it < P.n_iters; ++it) {
     // local step.  Pipeline over the CTA's cells, two barriers per cell:
     //   [elements(c) -> out; volume gradient(c), partial sums] | [vertices(c): gather out, volume
@@ -499,9 +502,11 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     // counts, [1] = ring offsets 0..5 (3 words) + m/h^2.
     F3 g = {0.f, 0.f, 0.f}, zv = {0.f, 0.f, 0.f};
     uint4 vr0;
+    // element results alternate between two buffers (rb, and ra, which is idle until the split),
+    // so the vertex phase of cell c and the element pass of cell c+1 share one barrier interval
     auto elements_and_gradient = [&](int cc) {
       const unsigned char* zcc = z4b + cc * cellz;
-      if (is_e) element_residual(ec_t, E, zcc, P, out_t);
+      if (is_e) element_residual(ec_t, E, zcc, P, reinterpret_cast<float4*>((cc & 1) ? rab : rbb) + tid);
       vr0 = P.vrole[2 * v];
       if (use_vol) {
         float S1 = 0.f, S2 = 0.f;
@@ -520,6 +525,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     __syncthreads();
     for (int c = 0; c < kact; ++c) {
       const unsigned char* zc = z4b + c * cellz;
+      const unsigned char* outb = (c & 1) ? rab : rbb;
       const int icnt = vr0.w & 0xff, rcnt = (vr0.w >> 8) & 0xff;
       F3 ev = {0.f, 0.f, 0.f};
       float S1, S2;
@@ -528,13 +534,13 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
 #pragma unroll
         for (int i = 0; i < kRegList; ++i) {
           if (i < icnt) {
-            const F3 o = lds3(rbb, (i & 1) ? (ioff[i >> 1] >> 16) : (ioff[i >> 1] & 0xffffu));
+            const F3 o = lds3(outb, (i & 1) ? (ioff[i >> 1] >> 16) : (ioff[i >> 1] & 0xffffu));
             ev = ev + o;
           }
         }
         if (icnt > kRegList) {
           const uint16_t* inc_tail = P.inc_off + P.inc_ptr[v];
-          for (int i = kRegList; i < icnt; ++i) ev = ev + lds3(rbb, inc_tail[i]);
+          for (int i = kRegList; i < icnt; ++i) ev = ev + lds3(outb, inc_tail[i]);
         }
       }
 
@@ -586,36 +592,33 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         }
         if (moved && isv) reinterpret_cast<float4*>(z4b + c * cellz)[v] = make_float4(zv.x, zv.y, zv.z, 0.f);
       }
-      if (isv) {
-        // right-hand side of the global step, r = e - (m/h^2) d with e including w_vol D; the
-        // -(m/h^2) d part was left in place by the previous update pass
-        const int m = 3 * c;
-        float* r0 = ra + fbase + ((m) & 7) * 16 + ((m) >> 3);
-        float* r1 = ra + fbase + ((m + 1) & 7) * 16 + ((m + 1) >> 3);
-        float* r2 = ra + fbase + ((m + 2) & 7) * 16 + ((m + 2) >> 3);
-        *r0 += fmaf(P.w_volume, D.x, ev.x);
-        *r1 += fmaf(P.w_volume, D.y, ev.y);
-        *r2 += fmaf(P.w_volume, D.z, ev.z);
-      }
-      __syncthreads();   // out consumed; right-hand side of cell c complete; z4 of cell c restored
-      if (c + 1 < kact) {
-        elements_and_gradient(c + 1);
-        __syncthreads();   // out(c+1) and the partial sums of cell c+1 complete
-      }
+      // elastic residual of the cell's vertices, e = sum of element results + w_vol D, parked in
+      // the owner's TMEM columns 32 + 3c .. (the fourth column written belongs to the next cell,
+      // which overwrites it later in this same pass)
+      tmem_st4(ta + 32 + 3 * c, fmaf(P.w_volume, D.x, ev.x), fmaf(P.w_volume, D.y, ev.y),
+               fmaf(P.w_volume, D.z, ev.z), 0.0f);
+      if (c + 1 < kact) elements_and_gradient(c + 1);
+      __syncthreads();   // out(c) consumed; out(c+1) and the partial sums of cell c+1 complete
     }
 
-    // split the right-hand sides into tf32 high and low parts (hi in place, lo over the dead
-    // element buffer), one float4 per thread and trip: conflict-free.  Round-to-nearest on the 13
-    // dropped mantissa bits; lo = x - hi is exact.
-    for (int q = tid; q < NP * 4; q += blockDim.x) {
-      const float4 x = reinterpret_cast<const float4*>(ra)[q];
-      float4 hi;
-      hi.x = __uint_as_float((__float_as_uint(x.x) + 0x1000u) & 0xffffe000u);
-      hi.y = __uint_as_float((__float_as_uint(x.y) + 0x1000u) & 0xffffe000u);
-      hi.z = __uint_as_float((__float_as_uint(x.z) + 0x1000u) & 0xffffe000u);
-      hi.w = __uint_as_float((__float_as_uint(x.w) + 0x1000u) & 0xffffe000u);
-      reinterpret_cast<float4*>(ra)[q] = hi;
-      reinterpret_cast<float4*>(rb)[q] = make_float4(x.x - hi.x, x.y - hi.y, x.z - hi.z, x.w - hi.w);
+    // right-hand sides of the global step, r = e - (m/h^2) d, split into tf32 high and low parts and
+    // written in mma A-fragment order (hi -> ra, lo -> rb; both element buffers are dead now).
+    // Round-to-nearest on the 13 dropped mantissa bits; lo = x - hi is exact.
+    {
+      float ee[16], dd[16];
+      tmem_ld16(ta + 32, ee);
+      tmem_ld16(ta + 16, dd);
+      const float nmh2 = -__uint_as_float(P.vrole[2 * v + 1].w);
+      if (isvp) {
+#pragma unroll
+        for (int m = 0; m < kRhs; ++m) {
+          const int idx = fbase + (m & 7) * 16 + (m >> 3);
+          const float x = m < 15 ? fmaf(nmh2, dd[m], ee[m]) : 0.0f;
+          const float hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+          ra[idx] = hi;
+          rb[idx] = x - hi;
+        }
+      }
     }
     __syncthreads();
 
@@ -674,10 +677,9 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     }
     __syncthreads();
 
-    // owner update: d += delta d, z = s + d, and -(m/h^2) d as the start of the next rhs
+    // owner update: d += delta d, z = s + d
     {
       float sv[16], dv[16];
-      const float nmh2 = -__uint_as_float(P.vrole[2 * v + 1].w);
       tmem_ld16(ta, sv);
       tmem_ld16(ta + 16, dv);
 #pragma unroll
@@ -688,8 +690,6 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           if (c < P.k)
             reinterpret_cast<float4*>(z4b)[c * NP + v] =
                 make_float4(sv[3 * c] + dv[3 * c], sv[3 * c + 1] + dv[3 * c + 1], sv[3 * c + 2] + dv[3 * c + 2], 0.f);
-#pragma unroll
-        for (int m = 0; m < 15; ++m) ra[fbase + (m & 7) * 16 + (m >> 3)] = nmh2 * dv[m];
       }
       tmem_st16(ta + 16, dv);
     }
@@ -697,28 +697,29 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   }
 
   // ---- epilogue: x_n+1 = x_n + (u0 + d), v_n+1 = (u0 + d)/h, staged in caller order through
-  //      shared memory so that the stores to pos / vel are coalesced
+  //      shared memory so that the loads of x_n and the stores to pos / vel are coalesced
   {
-    float dv[16], ur[16], xr[16];
+    float dv[16], ur[16];
     tmem_ld16(ta + 16, dv);
-    tmem_ld16(ta + 32, ur);
-    tmem_ld16(ta + 48, xr);
+    tmem_ld16(ta + 48, ur);
     float* const st = rb;                    // [2][3n]
     const int n3 = 3 * n;
     const float invh = 1.0f / h;
 #pragma unroll
     for (int c = 0; c < kMaxCellsPerCta; ++c) {
       if (c < kact) {
+        const size_t g = (size_t)(cell0 + c) * P.cell_stride;
+        for (int i = tid; i < n3; i += blockDim.x) st[i] = P.pos[g + i];
+        __syncthreads();
         if (isv) {
 #pragma unroll
           for (int q = 0; q < 3; ++q) {
             const float inc = ur[3 * c + q] + dv[3 * c + q];
-            st[vext3 + q] = xr[3 * c + q] + inc;
+            st[vext3 + q] += inc;
             st[n3 + vext3 + q] = inc * invh;
           }
         }
         __syncthreads();
-        const size_t g = (size_t)(cell0 + c) * P.cell_stride;
         for (int i = tid; i < n3; i += blockDim.x) { P.pos[g + i] = st[i]; P.vel[g + i] = st[n3 + i]; }
         __syncthreads();
       }
