@@ -216,6 +216,7 @@ def run_ours(args) -> None:
     import workloads as W
     from paper_2011_04332_b200 import NpfemHandle
     from paper_2011_04332_b200.harness import to_strided
+    from paper_2011_04332_b200.multi import max_over_ranks, rank_seed
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the npFEM path has no CPU fallback")
@@ -235,7 +236,7 @@ def run_ours(args) -> None:
     rest, tris = W.rest_shape(kind, level)
     mat = W.default_material(rest, tris)
     n, T = rest.shape[0], tris.shape[0]
-    rng = np.random.Generator(np.random.PCG64([spec["seed"], 0xCE11, rank]))
+    rng = np.random.Generator(np.random.PCG64(rank_seed(spec["seed"], rank)))
     radius = float(np.linalg.norm(rest, axis=1).max())
     rot, trans = W.random_rigid_placements(n_cells, spec["box"], radius, rng)
     pos0 = W.place_cells(rest, rot, trans)                                 # fp32 [N,V,3]
@@ -284,10 +285,7 @@ def run_ours(args) -> None:
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     per_launch_ms = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
     total_ms = ev[0].elapsed_time(ev[-1])
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dev)
     finite = bool(torch.isfinite(pos).all().item())
 
     # ---- end to end through the host-buffer entry point (pinned host memory)
@@ -304,10 +302,7 @@ def run_ours(args) -> None:
         h.step_host(n_cells, hp, hv, hf, n_iters)                          # blocking
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_e2e = float(t.item())
+    t_e2e = max_over_ranks(t_e2e, dev)
     field_bytes = n_cells * stride * 4
     if e2e_steps:
         e2e = {"value": world * n_cells * e2e_steps / t_e2e, "unit": "cell-steps/s",

@@ -456,3 +456,22 @@ def test_step_many_cells_matches_single_cell_calls():
     for i in range(5):
         pi, vi = c.step_cell(pos[i], vel[i], f[i], 4)
         assert np.array_equal(p[i], pi) and np.array_equal(v[i], vi)
+
+
+def test_oracle_reproduces_its_committed_config1_result():
+    """Regression guard of the oracle's own arithmetic: tests/golden/config1_oracle.txt was written
+    by tests/golden/make_golden.py from the oracle alone (the paper prints no value to cite).  A
+    change to the oracle that moves these numbers must name the passage or DESIGN.md reading that
+    justifies it and regenerate the file."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config1_oracle.txt")
+    ref = np.loadtxt(path)
+    w = W.make_config(1)
+    g = w.groups[0]
+    oc = O.OracleCell(g.tris, g.rest, g.material, w.dt)
+    pos, vel = oc.step(g.pos0, g.vel0, w.forces(0, 0), w.n_iters)
+    disp = pos[0] - g.pos0[0].astype(np.float64)
+    assert ref.shape == (g.rest.shape[0], 6)
+    scale = np.abs(ref[:, :3]).max()
+    assert np.abs(disp - ref[:, :3]).max() <= 1e-9 * scale      # fp64 summation-order slack
+    assert np.abs(vel[0] - ref[:, 3:]).max() <= 1e-9 * np.abs(ref[:, 3:]).max()
