@@ -492,9 +492,10 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const bool use_vol = P.w_volume > 0.0f;
   const float4* const ec_t = ecs + (is_e ? tid : 0);
   for (int it = 0; it < P.n_iters; ++it) {
-    // local step.  Pipeline over the CTA's cells, two barriers per cell:
-    //   [elements(c) -> out; volume gradient(c), partial sums] | [vertices(c): gather out, volume
-    //   multiplier, right-hand side] | [elements(c+1); ...] | ...
+    // local step.  Pipeline over the CTA's cells, one barrier per cell:
+    //   [elements(0) -> out B; volume gradient(0), partial sums] |
+    //   [vertices(c): gather out(c), volume multiplier, residual -> TMEM; elements(c+1) -> the other
+    //    out buffer; volume gradient(c+1), partial sums] | ...
     // The volume gradient only reads z, so every warp runs its share right after its elements:
     // warps that finish the element pass early keep working instead of waiting at the barrier.
     // Vertex-role constants (npfem_api.cu: vrole) are fetched just before they are needed instead
