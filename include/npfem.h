@@ -63,9 +63,10 @@ typedef struct {
                           /* l1 mass of a row stays <= inv_drop_tol * ||row||_1.  Default 2^-24     */
                           /* (below fp32 rounding of the kept sum); < 0 = that default;             */
                           /* 0 = keep everything (dense operator).                                  */
-  int volume_inner_iters; /* cap on the passes of the volume projection per local step (>= 1);     */
-                          /* default 2.  A pass is skipped once it cannot change the result at     */
-                          /* fp32 resolution (A-17); violations of several % need more   */
+  int volume_inner_iters; /* cap on the passes of the volume projection per local step (>= 1,      */
+                          /* <= 32); default 8.  The pass loop is adaptive: a pass is skipped once  */
+                          /* it cannot change the result at fp32 resolution (A-17), so    */
+                          /* near-rest cells take one pass whatever the cap                         */
   int cells_per_cta;      /* 1..5 cells share one CTA and every fetched operator block; 0 = auto   */
   int global_mode;        /* 0 = auto, 1 = fp32 SIMT blocks, 2 = 3xTF32 tensor-core blocks          */
   int pair_triangles;     /* local-step work items: 0 = auto / 1 = pairs of triangles across a shared */

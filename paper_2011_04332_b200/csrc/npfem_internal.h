@@ -87,9 +87,10 @@ int build_plan(int n_verts, int n_tris, const int32_t* tris, const double* rest_
 // Shared-memory carve-up used by both the host (to size the launch) and the kernel.
 //   z4   [k][NP] float4   current iterate z = s + d, cell-local coordinates (w unused)
 //   ec   [9][E] float4    element constants (kElemGroups groups of 4 words, see npfem_api.cu)
-//   ra   [nvb][32] float4 right-hand sides in mma A-fragment order (fp32 while the local step
-//                         accumulates them, then their tf32 high parts)
-//   rb   max(E*64, NP*64) element results `out` [4][E] float4 during the local step, then the
+//   ra   max(E*64, NP*64) element results `out` [4][E] float4 of the ODD cells during the local
+//                         step, then the tf32 high parts of the right-hand sides in mma
+//                         A-fragment order ([nvb][32] float4)
+//   rb   max(E*64, NP*64) element results of the EVEN cells during the local step, then the
 //                         tf32 low parts of the right-hand sides, then the increments of d
 //   red  [5][32] float4   per-warp partial sums of the volume reductions
 // The inertial prediction s and the correction d are private to the thread that owns the vertex
@@ -105,9 +106,9 @@ inline SmemLayout smem_layout(int n, int E, int nvb, int k) {
   int off = 0;
   L.z4 = off; off += k * NP * 16;
   L.ec = off; off += kElemGroups * E * 16;
-  L.ra = off; off += NP * 64;
-  int rb = E * 64 > NP * 64 ? E * 64 : NP * 64;
-  L.rb = off; off += rb;
+  const int rbuf = E * 64 > NP * 64 ? E * 64 : NP * 64;   // both buffers hold [4][E] element results
+  L.ra = off; off += rbuf;
+  L.rb = off; off += rbuf;
   L.red = off; off += kMaxCellsPerCta * 32 * 16;
   L.total = off;
   return L;

@@ -137,8 +137,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     o.global_mode = opts->global_mode;
     o.pair_triangles = opts->pair_triangles;
   }
-  if (o.volume_inner_iters <= 0) o.volume_inner_iters = 2;
-  if (o.volume_inner_iters > 8) o.volume_inner_iters = 8;
+  if (o.volume_inner_iters <= 0) o.volume_inner_iters = 8;
+  if (o.volume_inner_iters > 32) o.volume_inner_iters = 32;
   if (o.cells_per_cta < 0 || o.cells_per_cta > kMaxCellsPerCta)
     return fail(NPFEM_EINVAL, "cells_per_cta must be 0..5");
   if (o.global_mode < 0 || o.global_mode > 2) return fail(NPFEM_EINVAL, "global_mode must be 0..2");
