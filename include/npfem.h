@@ -127,6 +127,17 @@ int npfem_destroy(npfem_handle h);
 const char* npfem_last_error(void); /* thread-local, static storage; never NULL                   */
 int npfem_cell_stride(npfem_handle h); /* floats per cell actually used                           */
 
+/*
+ * npfem_measure_fp32_peak: same-run measurement of the FP32 pipe rate that bounds the step kernel
+ * (SURVEY.md 8(d) asks for a measured FMA peak beside the nominal one).
+ * Runs a register-resident arithmetic loop on every SM of the current device and returns the best
+ * of 4 timed launches (CUDA events) in TFLOP/s.  Blocking; allocates 4 bytes for its own use.
+ *   variant  0 = FFMA (2 flop), 1 = packed FFMA2 (4 flop), 2 = FADD (1 flop),
+ *            3 = FFMA and FADD alternating (1.5 flop per instruction on average)
+ *   out_tflops  host, receives the rate.  Errors: NPFEM_EINVAL, NPFEM_ECUDA.
+ */
+int npfem_measure_fp32_peak(int variant, double* out_tflops);
+
 /* Introspection of a handle (all host-side, cheap): what the create step decided.               */
 typedef struct {
   int n_verts, n_tris, n_hinges;

@@ -6,8 +6,8 @@ device raises.
 """
 from .binding import (NpfemError, NpfemHandle, NpfemPlan, load_library, npfem_create,
                       npfem_destroy, npfem_step, npfem_step_host, npfem_last_error,
-                      npfem_cell_stride, MATERIAL_FIELDS, QUERY)
+                      npfem_cell_stride, npfem_measure_fp32_peak, MATERIAL_FIELDS, QUERY)
 
 __all__ = ["NpfemError", "NpfemHandle", "NpfemPlan", "load_library", "npfem_create",
            "npfem_destroy", "npfem_step", "npfem_step_host", "npfem_last_error",
-           "npfem_cell_stride", "MATERIAL_FIELDS", "QUERY"]
+           "npfem_cell_stride", "npfem_measure_fp32_peak", "MATERIAL_FIELDS", "QUERY"]

@@ -84,9 +84,18 @@ def load_library(path: str | None = None):
     lib.npfem_plan_info.argtypes = [vp, C.POINTER(Info)]
     lib.npfem_plan_query.restype = C.c_int
     lib.npfem_plan_query.argtypes = [vp, C.c_int, vp, C.c_int]
+    lib.npfem_measure_fp32_peak.restype = C.c_int
+    lib.npfem_measure_fp32_peak.argtypes = [C.c_int, dp]
     if path is None:
         _lib = lib
     return lib
+
+
+def npfem_measure_fp32_peak(variant: int = 0) -> float:
+    """TFLOP/s of the FP32 pipe on the current device (0 FFMA, 1 FFMA2, 2 FADD, 3 FFMA+FADD)."""
+    out = C.c_double(0.0)
+    _check(load_library().npfem_measure_fp32_peak(int(variant), C.byref(out)))
+    return float(out.value)
 
 
 def npfem_last_error() -> str:
