@@ -41,16 +41,21 @@ N_FORCE_FIELDS = 4          # pre-generated per-step force fields, cycled (each 
 # nnz of the nested-dissection Cholesky factor of A_sys per icosphere level
 NNZ_L = {42: 573, 162: 4620, 642: 31397}
 FLOP_PER_TRI = 210          # F, 2x2 SVD via F^T F, strain clamp, area hyperbola (4 Newton steps), G^T P
+FLOP_PER_NEWTON = 23        # one Newton step on the hyperbola stationarity (g, g', quotient, update)
 FLOP_PER_HINGE = 60         # k = sum K_i x_i, normalise, scatter 4 x 3
 FLOP_VOL_PER_TRI, FLOP_VOL_PER_VERT, VOL_INNER = 45, 15, 2
 FLOP_RHS_PER_VERT = 10
 
 
-def flops_per_cell_iteration(n_verts: int, n_tris: int) -> float:
+def flops_per_cell_iteration(n_verts: int, n_tris: int, vol_passes: int = VOL_INNER,
+                             newton_steps: int = 4) -> float:
+    """Algorithmic flops of one local/global iteration of one cell (defaults: the count DESIGN.md
+    states).  vol_passes / newton_steps let the caller count what the kernel really executes on
+    a near-rest suspension: one volume pass and one Newton step per triangle (A-17, A-18)."""
     n_h = 3 * n_tris // 2
     nnz_l = NNZ_L.get(n_verts, int(49 * n_verts))
-    local = FLOP_PER_TRI * n_tris + FLOP_PER_HINGE * n_h
-    volume = VOL_INNER * (FLOP_VOL_PER_TRI * n_tris + FLOP_VOL_PER_VERT * n_verts)
+    local = (FLOP_PER_TRI - (4 - newton_steps) * FLOP_PER_NEWTON) * n_tris + FLOP_PER_HINGE * n_h
+    volume = vol_passes * (FLOP_VOL_PER_TRI * n_tris + FLOP_VOL_PER_VERT * n_verts)
     solve = 12 * nnz_l + 6 * n_verts            # 3 rhs x (forward + backward) x 2 flop per entry
     return float(local + volume + solve + FLOP_RHS_PER_VERT * n_verts)
 
@@ -62,19 +67,25 @@ def hbm_bytes_per_cell_step(n_verts: int) -> int:
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x FMA x max clock
 
 
+TRAFFIC_CAPTURE = "r2_dram_traffic.csv"     # newest committed `ncu --set full` capture (profiles/)
+
+
 def measured_dram_traffic(n_verts: int, n_cells: int):
-    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the step kernel,
-    from the committed `ncu --set full` capture: profiles/r1c_dram_traffic.csv holds the bytes per
-    cell measured there; a launch moves that times its cells.  None without a capture."""
-    path = os.path.join(ROOT, "profiles", "r1c_dram_traffic.csv")
+    """(DRAM bytes per launch, provenance) of the step kernel: dram__bytes_read.sum +
+    dram__bytes_write.sum from the newest committed `ncu --set full` capture.  The csv holds the
+    bytes per cell measured there and the commit of the kernel it was taken on; a launch moves
+    that times its cells.  (None, reason) without a capture for this mesh size."""
+    path = os.path.join(ROOT, "profiles", TRAFFIC_CAPTURE)
     if not os.path.exists(path):
-        return None
+        return None, "no capture committed"
     with open(path) as fh:
         rows = [ln.strip().split(",") for ln in fh if ln.strip() and not ln.startswith("#")]
     rec = dict(zip(rows[0], rows[1]))
     if int(rec["n_verts"]) != n_verts:
-        return None
-    return float(rec["dram_bytes_per_cell"]) * n_cells
+        return None, "capture is for another mesh size"
+    return float(rec["dram_bytes_per_cell"]) * n_cells, (
+        f"profiles/{TRAFFIC_CAPTURE}: {rec['dram_bytes_per_cell']} B per cell at "
+        f"{rec.get('n_cells', '?')} cells, kernel of commit {rec.get('commit', '?')}")
 
 
 def load_peaks() -> dict:
@@ -210,11 +221,89 @@ def run_reference(args) -> None:
 
 
 # ---- the CUDA arm -------------------------------------------------------------------------------
+def roofline_of(n, T, n_iters, n_cells, launch_ms, peak_measured, peaks, clocks=None, traffic=True):
+    """Roofline object of the fused step kernel for one workload: the path is
+    bound by plain FP32 issue, so achieved = algorithmic flops per launch / launch duration, against
+    the FFMA rate measured in this run (npfem_measure_fp32_peak) and, for reference, the nominal one."""
+    f_alg = flops_per_cell_iteration(n, T) * n_iters * n_cells
+    f_exe = flops_per_cell_iteration(n, T, vol_passes=1, newton_steps=1) * n_iters * n_cells
+    b_alg = hbm_bytes_per_cell_step(n) * n_cells
+    sec = launch_ms * 1e-3
+    achieved = f_alg / sec / 1e12
+    r = {"bound": "alu", "achieved": achieved, "peak": peak_measured, "unit": "TFLOP/s",
+         "frac": achieved / peak_measured, "kernel": "npfem_step_kernel",
+         "peak_source": "measured in this run: npfem_measure_fp32_peak(FFMA), best of 4 launches",
+         "peak_measured": peak_measured, "peak_nominal": FP32_PEAK_TFLOPS_NOMINAL,
+         "frac_of_nominal": achieved / FP32_PEAK_TFLOPS_NOMINAL,
+         "peak_nominal_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz",
+         "algorithmic_flops_per_launch": f_alg, "launch_ms": launch_ms,
+         "executed_equivalent": {
+             "flops_per_launch": f_exe, "achieved": f_exe / sec / 1e12,
+             "frac": f_exe / sec / 1e12 / peak_measured,
+             "note": "the same count with the 1 volume pass and 1 area-Newton step per triangle "
+                     "that the adaptive loops really take on a near-rest suspension (A-17, A-18); "
+                     "the algorithmic count charges 2 passes and 4 steps"},
+         "hbm": {"achieved_gbs": b_alg / sec / 1e9, "peak_gbs": peaks["hbm_gbs"],
+                 "frac": b_alg / sec / 1e9 / peaks["hbm_gbs"], "peak_source": peaks["source"],
+                 "algorithmic_bytes_per_launch": b_alg}}
+    if traffic:
+        r["traffic"], r["traffic_source"] = measured_dram_traffic(n, n_cells)
+    if clocks and clocks.get("sm_mhz"):
+        at_clock = 148 * 128 * 2 * clocks["sm_mhz"] * 1e6 / 1e12
+        r["frac_at_observed_clock"] = achieved / at_clock
+    return r
+
+
+def time_extra_workload(W, NpfemHandle, to_strided, dev, name, kind, level, n_cells, n_iters,
+                        force_kind, seed, steps, warmup, peak_measured, peaks):
+    """Device-resident timing of one non-headline workload (other cell types / config 5)."""
+    import torch
+    rest, tris = W.rest_shape(kind, level)
+    mat = W.default_material(rest, tris)
+    n, T = rest.shape[0], tris.shape[0]
+    rng = np.random.Generator(np.random.PCG64(seed))
+    radius = float(np.linalg.norm(rest, axis=1).max())
+    rot, trans = W.random_rigid_placements(n_cells, 300.0, radius, rng)
+    pos0 = W.place_cells(rest, rot, trans)
+    h = NpfemHandle(tris, rest, mat, W.configs.DT, 0, n_cells)
+    stride = h.cell_stride
+    pos = to_strided(pos0, stride, dev)
+    vel = torch.zeros_like(pos)
+    f = torch.zeros((n_cells, stride), dtype=torch.float32, device=dev)
+    if force_kind == "caps":        # config 5: +-20 pN on the two diametric caps, constant in time
+        fc = W.forces.cap_pull_forces(rest, rot, 20e-3)
+        f[:, : 3 * n] = torch.as_tensor(fc.reshape(n_cells, 3 * n), device=dev)
+    else:
+        f[:, : 3 * n] = W.forces.gaussian_forces_torch((n_cells, 3 * n), 1e-3, seed, 0, dev)
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        h.step(n_cells, pos, vel, f, n_iters, stream)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(steps):
+        h.step(n_cells, pos, vel, f, n_iters, stream)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / steps
+    info = h.info()
+    finite = bool(torch.isfinite(pos).all().item())
+    del h, pos, vel, f
+    torch.cuda.empty_cache()
+    r = roofline_of(n, T, n_iters, n_cells, ms, peak_measured, peaks, traffic=False)
+    return {"workload": name, "n_cells": n_cells, "n_verts": n, "n_iters": n_iters, "steps": steps,
+            "warmup": warmup, "ms_per_step": ms, "cell_steps_per_s": n_cells / (ms * 1e-3),
+            "vertex_iterations_per_s": n_cells * n * n_iters / (ms * 1e-3),
+            "cells_per_cta": info["cells_per_cta"], "threads_per_cta": info["threads_per_cta"],
+            "frac": r["frac"], "frac_executed_equivalent": r["executed_equivalent"]["frac"],
+            "achieved_tflops": r["achieved"], "hbm_frac": r["hbm"]["frac"], "state_finite": finite}
+
+
 def run_ours(args) -> None:
     import torch
     import torch.distributed as dist
     import workloads as W
-    from paper_2011_04332_b200 import NpfemHandle
+    from paper_2011_04332_b200 import NpfemHandle, npfem_measure_fp32_peak
     from paper_2011_04332_b200.harness import to_strided
     from paper_2011_04332_b200.multi import max_over_ranks, rank_seed
 
@@ -227,6 +316,13 @@ def run_ours(args) -> None:
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+
+    # ---- the roofline denominator, measured on this GPU before the timed region
+    peak_measured = npfem_measure_fp32_peak(0)
+    peak_variants = {"ffma": peak_measured}
+    if rank == 0 and not args.kernel_only:
+        peak_variants.update({"ffma2": npfem_measure_fp32_peak(1), "fadd": npfem_measure_fp32_peak(2),
+                              "ffma_fadd_mix": npfem_measure_fp32_peak(3)})
 
     # ---- workload: config 4, this rank's own cells (weak scaling: fixed cells per GPU)
     spec = W.CONFIGS[CONFIG_ID]
@@ -288,27 +384,29 @@ def run_ours(args) -> None:
     total_ms = max_over_ranks(total_ms, dev)
     finite = bool(torch.isfinite(pos).all().item())
 
-    # ---- end to end through the host-buffer entry point (pinned host memory)
+    # ---- end to end through the host-buffer entry point (pinned host memory): every step copies
+    #      pos / vel / that step's own force field host -> device and pos / vel back
     e2e = None
-    e2e_steps = 0 if args.kernel_only else max(1, min(args.steps, 3))
-    hp = to_strided(pos0, stride, "cpu").pin_memory()
-    hv = torch.zeros_like(hp).pin_memory()
-    hf = fields[0].cpu().pin_memory()
-    if e2e_steps:
-        h.step_host(n_cells, hp, hv, hf, n_iters)                          # warm-up: staging ring
-    barrier()
-    t0 = time.perf_counter()
-    for s in range(e2e_steps):
-        h.step_host(n_cells, hp, hv, hf, n_iters)                          # blocking
-    torch.cuda.synchronize()
-    t_e2e = time.perf_counter() - t0
-    t_e2e = max_over_ranks(t_e2e, dev)
+    e2e_steps = 0 if args.kernel_only else max(1, min(args.steps, 10))
     field_bytes = n_cells * stride * 4
     if e2e_steps:
+        hp = to_strided(pos0, stride, "cpu").pin_memory()
+        hv = torch.zeros_like(hp).pin_memory()
+        hfs = [f.cpu().pin_memory() for f in fields]
+        h.step_host(n_cells, hp, hv, hfs[0], n_iters)                      # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for s in range(e2e_steps):
+            h.step_host(n_cells, hp, hv, hfs[(s + 1) % len(hfs)], n_iters)  # blocking
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        t_e2e = max_over_ranks(t_e2e, dev)
         e2e = {"value": world * n_cells * e2e_steps / t_e2e, "unit": "cell-steps/s",
                "h2d_bytes_per_step": 3 * field_bytes, "d2h_bytes_per_step": 2 * field_bytes,
                "steps": e2e_steps, "ms_per_step": 1e3 * t_e2e / e2e_steps,
+               "force_fields_cycled": len(hfs),
                "api": "npfem_step_host (pinned host buffers, chunked 3-stream pipeline)"}
+        del hp, hv, hfs
 
     if rank != 0:
         if world > 1:
@@ -318,20 +416,21 @@ def run_ours(args) -> None:
     # ---- roofline of the fused step kernel (the only kernel of a step)
     peaks = load_peaks()
     launch_ms = statistics.mean(per_launch_ms)
-    f_alg = flops_per_cell_iteration(n, T) * n_iters * n_cells
-    b_alg = hbm_bytes_per_cell_step(n) * n_cells
-    achieved_tflops = f_alg / (launch_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "achieved": achieved_tflops, "peak": FP32_PEAK_TFLOPS_NOMINAL,
-                "unit": "TFLOP/s", "frac": achieved_tflops / FP32_PEAK_TFLOPS_NOMINAL,
-                "traffic": measured_dram_traffic(n, n_cells), "kernel": "npfem_step_kernel",
-                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
-                "algorithmic_flops_per_launch": f_alg, "launch_ms": launch_ms,
-                "hbm": {"achieved_gbs": b_alg / (launch_ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
-                        "frac": b_alg / (launch_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                        "peak_source": peaks["source"], "algorithmic_bytes_per_launch": b_alg}}
-    if clocks and clocks.get("sm_mhz"):
-        at_clock = 148 * 128 * 2 * clocks["sm_mhz"] * 1e6 / 1e12
-        roofline["frac_at_observed_clock"] = achieved_tflops / at_clock
+    roofline = roofline_of(n, T, n_iters, n_cells, launch_ms, peak_measured, peaks, clocks)
+    roofline["fp32_pipe_tflops_measured"] = peak_variants
+
+    # ---- the other cell types and the large-deformation config through the same kernel
+    #      (not the headline: BASELINE.json configs 3 and 5; SURVEY.md H8 many-small-cells packing)
+    others = []
+    if world == 1 and not args.kernel_only and not args.cells:
+        del pos, vel, fields, h
+        torch.cuda.empty_cache()
+        for name, kind2, level2, nc2, it2, fk in (
+                ("400000 PLT-1 cells (42 vertices), 20 iterations, N(0,(1 pN)^2) forces", "plt", 1, 400000, 20, "gauss"),
+                ("200000 RBC-2 cells (162 vertices), 20 iterations, N(0,(1 pN)^2) forces", "rbc", 2, 200000, 20, "gauss"),
+                ("config5: 20000 RBC-3 cells, 30 iterations, +-20 pN cap pulls (first steps of the stretch)", "rbc", 3, 20000, 30, "caps")):
+            others.append(time_extra_workload(W, NpfemHandle, to_strided, dev, name, kind2, level2, nc2,
+                                              it2, fk, 900 + len(others), 5, 3, peak_measured, peaks))
 
     cpu = time_oracle(budget_s=12.0, steps=1) if world == 1 and not args.kernel_only else None
     value = world * n_cells * args.steps / (total_ms * 1e-3)
@@ -351,6 +450,8 @@ def run_ours(args) -> None:
                        "l2": "inputs (2.3 GB per step) exceed L2; no flush needed"},
             "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "clocks": clocks,
             "state_finite": finite}
+    if others:
+        line["other_workloads"] = others
     if cpu is not None:
         line["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
     print(json.dumps(line))

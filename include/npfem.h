@@ -84,8 +84,11 @@ typedef struct {
  *   dt               time step h > 0
  *   cell_stride_floats  floats between consecutive cells in pos/vel/fext; >= 3*n_verts; 0 = the
  *                    default padded stride (3*n_verts rounded up to a multiple of 4)
- *   max_cells        upper bound on n_cells of any later npfem_step (sizes nothing today; kept so
- *                    that npfem_step never allocates whatever the implementation)
+ *   max_cells        upper bound on n_cells of any later npfem_step / npfem_step_host call; > 0:
+ *                    the bound is enforced (NPFEM_EINVAL beyond it) and the streams and the
+ *                    device staging ring of npfem_step_host are allocated now (3 stages x 3 fields
+ *                    x min(max_cells, ~32 MB worth of cells)), so that no step entry point ever
+ *                    allocates; 0: no bound, npfem_step_host sizes its ring on first use
  *   opts             host, may be NULL
  *   out              receives the handle; the handle owns all device memory it allocates
  * Errors: NPFEM_EINVAL, NPFEM_ENOMEM, NPFEM_ELIMIT, NPFEM_ECUDA (also when no CUDA device exists:
@@ -114,8 +117,9 @@ int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float*
 /*
  * npfem_step_host: the same step with HOST buffers (pinned or pageable): cells are cut into
  * chunks that flow host->device, through the step kernel and device->host on three streams so
- * copies overlap compute.  Blocking: returns when pos/vel hold the new state.  Uses a device
- * staging ring owned by the handle (allocated on first use, reused afterwards).
+ * copies overlap compute.  Blocking: returns when pos/vel hold the new state (also on error: no
+ * copy is left in flight).  Uses the device staging ring owned by the handle (allocated by
+ * npfem_create when max_cells > 0, else on first use).
  *   pos, vel  host, float, in/out, [n_cells][cell_stride];  fext host, in
  * Bytes moved per call: 3 fields in, 2 fields out, n_cells*cell_stride*4 bytes each.
  */

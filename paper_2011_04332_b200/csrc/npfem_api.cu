@@ -66,6 +66,60 @@ void fill_info(const Plan& P, int cell_stride, npfem_info* o) {
 
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Makes the handle's device current for the lifetime of the guard (the handle's tables, streams
+// and staging ring live on the device that was current in npfem_create).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(int device) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != device) {
+      err = cudaSetDevice(device);
+      switched = err == cudaSuccess;
+    }
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
+void destroy_pipeline(npfem_handle_s* h) {
+  for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
+    for (int f = 0; f < 3; ++f) {
+      if (h->stage[sidx][f]) cudaFree(h->stage[sidx][f]);
+      h->stage[sidx][f] = nullptr;
+    }
+    if (h->streams[sidx]) cudaStreamDestroy(h->streams[sidx]);
+    h->streams[sidx] = nullptr;
+  }
+  h->pipeline_ready = false;
+}
+
+// Streams and device staging ring of npfem_step_host: chunks of a whole number of CTAs' worth of
+// cells, about 32 MB per field, never more than `cells_hint` cells (0 = no hint).  Everything
+// created so far is released again when a later allocation fails.
+int create_pipeline(npfem_handle_s* h, int cells_hint) {
+  if (h->pipeline_ready) return NPFEM_OK;
+  const size_t cell_bytes = (size_t)h->cell_stride * sizeof(float);
+  const int k = h->plan.cells_per_cta;
+  int chunk = (int)((32u << 20) / cell_bytes);
+  if (cells_hint > 0 && chunk > cells_hint) chunk = cells_hint;
+  chunk = (chunk + k - 1) / k * k;
+  if (chunk < k) chunk = k;
+  h->chunk_cells = chunk;
+  for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
+    cudaError_t e = cudaStreamCreateWithFlags(&h->streams[sidx], cudaStreamNonBlocking);
+    if (e != cudaSuccess) { h->streams[sidx] = nullptr; destroy_pipeline(h); return cuda_err(e, "cudaStreamCreate"); }
+    for (int f = 0; f < 3; ++f) {
+      e = cudaMalloc(&h->stage[sidx][f], (size_t)chunk * cell_bytes);
+      if (e != cudaSuccess) { h->stage[sidx][f] = nullptr; destroy_pipeline(h); return cuda_err(e, "cudaMalloc(staging ring)"); }
+    }
+  }
+  h->pipeline_ready = true;
+  return NPFEM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -260,6 +314,10 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.blk_col = reinterpret_cast<const uint16_t*>(base + secs[10].off);
   D.blk_val = reinterpret_cast<const float*>(base + secs[11].off);
   D.L = smem_layout(n, E, P.nvb, P.cells_per_cta);
+  if (max_cells > 0) {   // everything any later step entry point needs exists now
+    rc = create_pipeline(H, max_cells);
+    if (rc != NPFEM_OK) { cudaFree(H->blob); delete H; return rc; }
+  }
   *out = H;
   return NPFEM_OK;
 }
@@ -281,6 +339,9 @@ int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float*
   if (n_cells < 0 || n_iters < 0) return set_err(NPFEM_EINVAL, "negative n_cells or n_iters");
   if (n_cells == 0) return NPFEM_OK;
   if (!pos || !vel || !fext) return set_err(NPFEM_EINVAL, "null device pointer");
+  if (h->max_cells > 0 && n_cells > h->max_cells) return set_err(NPFEM_EINVAL, "n_cells exceeds the max_cells given to npfem_create");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_err(guard.err, "cudaSetDevice(handle device)");
   DevParams p = h->dev;
   p.n_cells = n_cells; p.n_iters = n_iters;
   p.pos = pos; p.vel = vel; p.fext = fext;
@@ -296,59 +357,52 @@ int npfem_step_host(npfem_handle h, int n_cells, float* pos, float* vel, const f
   if (n_cells < 0 || n_iters < 0) return set_err(NPFEM_EINVAL, "negative n_cells or n_iters");
   if (n_cells == 0) return NPFEM_OK;
   if (!pos || !vel || !fext) return set_err(NPFEM_EINVAL, "null host pointer");
+  if (h->max_cells > 0 && n_cells > h->max_cells) return set_err(NPFEM_EINVAL, "n_cells exceeds the max_cells given to npfem_create");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_err(guard.err, "cudaSetDevice(handle device)");
   const size_t cell_bytes = (size_t)h->cell_stride * sizeof(float);
-  cudaError_t e;
-  if (!h->pipeline_ready) {
-    // chunk = a whole number of CTAs' worth of cells, about 32 MB per field
-    int chunk = (int)((32u << 20) / cell_bytes);
-    chunk = chunk / h->plan.cells_per_cta * h->plan.cells_per_cta;
-    if (chunk < h->plan.cells_per_cta) chunk = h->plan.cells_per_cta;
-    h->chunk_cells = chunk;
-    for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
-      e = cudaStreamCreateWithFlags(&h->streams[sidx], cudaStreamNonBlocking);
-      if (e != cudaSuccess) return cuda_err(e, "cudaStreamCreate");
-      for (int f = 0; f < 3; ++f) {
-        e = cudaMalloc(&h->stage[sidx][f], (size_t)chunk * cell_bytes);
-        if (e != cudaSuccess) return cuda_err(e, "cudaMalloc(staging)");
-      }
-    }
-    h->pipeline_ready = true;
+  if (!h->pipeline_ready) {   // handle created with max_cells = 0: the ring is sized on first use
+    int rc = create_pipeline(h, 0);
+    if (rc != NPFEM_OK) return rc;
   }
   const int chunk = h->chunk_cells;
-  int idx = 0;
-  for (int c0 = 0; c0 < n_cells; c0 += chunk, ++idx) {
+  cudaError_t e = cudaSuccess;
+  int rc = NPFEM_OK, idx = 0;
+  const char* what = "";
+  for (int c0 = 0; c0 < n_cells && rc == NPFEM_OK && e == cudaSuccess; c0 += chunk, ++idx) {
     const int sidx = idx % npfem_handle_s::kStages;
     const int nc = (n_cells - c0 < chunk) ? (n_cells - c0) : chunk;
     const size_t off = (size_t)c0 * h->cell_stride, bytes = (size_t)nc * cell_bytes;
     cudaStream_t st = h->streams[sidx];
     // stream order serialises reuse of this stage's buffers with its previous chunk
+    what = "cudaMemcpyAsync(H2D)";
     e = cudaMemcpyAsync(h->stage[sidx][0], pos + off, bytes, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h->stage[sidx][1], vel + off, bytes, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h->stage[sidx][2], fext + off, bytes, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return cuda_err(e, "cudaMemcpyAsync(H2D)");
-    int rc = npfem_step(h, nc, h->stage[sidx][0], h->stage[sidx][1], h->stage[sidx][2], n_iters, st);
-    if (rc != NPFEM_OK) return rc;
+    if (e != cudaSuccess) break;
+    rc = npfem_step(h, nc, h->stage[sidx][0], h->stage[sidx][1], h->stage[sidx][2], n_iters, st);
+    if (rc != NPFEM_OK) break;
+    what = "cudaMemcpyAsync(D2H)";
     e = cudaMemcpyAsync(pos + off, h->stage[sidx][0], bytes, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(vel + off, h->stage[sidx][1], bytes, cudaMemcpyDeviceToHost, st);
-    if (e != cudaSuccess) return cuda_err(e, "cudaMemcpyAsync(D2H)");
   }
+  // success or not, nothing may still be writing into the caller's buffers when this returns
   for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
-    e = cudaStreamSynchronize(h->streams[sidx]);
-    if (e != cudaSuccess) return cuda_err(e, "cudaStreamSynchronize");
+    cudaError_t es = cudaStreamSynchronize(h->streams[sidx]);
+    if (e == cudaSuccess && rc == NPFEM_OK && es != cudaSuccess) { e = es; what = "cudaStreamSynchronize"; }
   }
+  if (rc != NPFEM_OK) return rc;
+  if (e != cudaSuccess) return cuda_err(e, what);
   return NPFEM_OK;
 }
 
 int npfem_destroy(npfem_handle h) {
   if (!h) return NPFEM_OK;
-  if (h->pipeline_ready) {
-    for (int sidx = 0; sidx < npfem_handle_s::kStages; ++sidx) {
-      for (int f = 0; f < 3; ++f)
-        if (h->stage[sidx][f]) cudaFree(h->stage[sidx][f]);
-      if (h->streams[sidx]) cudaStreamDestroy(h->streams[sidx]);
-    }
+  {
+    DeviceGuard guard(h->device);
+    destroy_pipeline(h);
+    if (h->blob) cudaFree(h->blob);
   }
-  if (h->blob) cudaFree(h->blob);
   delete h;
   return NPFEM_OK;
 }
