@@ -17,8 +17,11 @@
  *    and parameters.
  *  - BASELINE.json north_star: local step = projection of every triangle's strain, bending hinge
  *    and area/volume constraint; global step = solve (M/h^2 + sum w A^T A) x = rhs.
+ *  - PAPER.md:60 ("with minor modifications of equation (2), one can readily simulate a
+ *    viscoelastic material"), :145, :183 (parameters Calpha, Cbeta): Rayleigh damping
+ *    f_d = -(c_alpha M + c_beta L_el) v, integrated implicitly (reading A-20).
  * The paper prints none of the energies; every formula below is a READING listed in DESIGN.md
- * (A-1 ... A-16).  Agreement with the real npFEM code is
+ * (A-1 ... A-20).  Agreement with the real npFEM code is
  * "parity unpinned"; what IS pinned (tests/test_oracle_pins.py) are invariants, closed forms,
  * library routines and brute force.
  *
@@ -63,6 +66,7 @@ typedef struct oracle_cell {
   double *w_h;     /* [H] hinge weights */
   double *r_h;     /* [H] rest magnitudes ||sum K_i X_i|| */
   double V0;       /* rest volume */
+  double *Lel;     /* dense elastic Laplacian sum_t (w_s+w_a) G^T G + sum_h w_h K^T K [n][n] */
   double *A;       /* dense A_sys [n][n] */
   double *L;       /* dense lower Cholesky factor of A_sys [n][n] */
   double *LT;      /* its transpose, so that the backward substitution also reads rows */
@@ -306,7 +310,7 @@ static int chol_dense(int n, const double *A, double *L) {
 void oracle_destroy(oracle_cell *c) {
   if (!c) return;
   free(c->tris); free(c->X); free(c->G); free(c->area); free(c->mass); free(c->hinge);
-  free(c->K); free(c->w_h); free(c->r_h); free(c->A); free(c->L); free(c->LT); free(c);
+  free(c->K); free(c->w_h); free(c->r_h); free(c->Lel); free(c->A); free(c->L); free(c->LT); free(c);
 }
 
 int oracle_create(int n, int T, const int32_t *tris, const double *X, const oracle_material *mat,
@@ -315,7 +319,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   *out = NULL;
   if (n < 4 || T < 4 || !tris || !X || !mat || !(h > 0)) return ORACLE_EINVAL;
   if (mat->s_min > mat->s_max || mat->a_min > mat->a_max || mat->v_min > mat->v_max) return ORACLE_EINVAL;
-  if (mat->c_alpha != 0.0 || mat->c_beta != 0.0) return ORACLE_EINVAL;          /* A-5 */
+  if (mat->c_alpha < 0.0 || mat->c_beta < 0.0) return ORACLE_EINVAL;
   if (!(mat->cell_mass > 0)) return ORACLE_EINVAL;
   for (int i = 0; i < 3*T; ++i) if (tris[i] < 0 || tris[i] >= n) return ORACLE_EINVAL;
   if ((3*T) % 2) return ORACLE_EINVAL;
@@ -333,6 +337,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   c->K = (double*)malloc(sizeof(double)*4*H);
   c->w_h = (double*)malloc(sizeof(double)*H);
   c->r_h = (double*)malloc(sizeof(double)*H);
+  c->Lel = (double*)calloc((size_t)n*n, sizeof(double));
   c->A = (double*)calloc((size_t)n*n, sizeof(double));
   c->L = (double*)malloc(sizeof(double)*(size_t)n*n);
   c->LT = (double*)malloc(sizeof(double)*(size_t)n*n);
@@ -414,21 +419,27 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   c->V0 = oracle_volume(T, tris, X);
   if (!(c->V0 > 0)) { oracle_destroy(c); return ORACLE_EINVAL; }
 
-  /* step 5: A_sys = diag(m)/h^2 + sum_t (w_s+w_a) G^T G + sum_h w_h K^T K + w_volume I */
-  for (int v = 0; v < n; ++v) c->A[(size_t)v*n+v] += c->mass[v] / (h*h) + mat->w_volume;
+  /* step 5: L_el = sum_t (w_s+w_a) G^T G + sum_h w_h K^T K;
+   *         A_sys = (1/h^2 + c_alpha/h) diag(m) + (1 + c_beta/h) L_el + w_volume I
+   * (c_alpha = c_beta = 0: the undamped system of SURVEY.md 8(c); otherwise reading A-20: the
+   * Rayleigh damping force -(c_alpha M + c_beta L_el)(x - x_n)/h of implicit Euler moves
+   * (c_alpha M + c_beta L_el)/h to the left-hand side) */
   for (int t = 0; t < T; ++t) {
     double w = (mat->k_strain + mat->k_area) * c->area[t];
     const double *G = c->G + 6*t;
     for (int p = 0; p < 3; ++p)
       for (int q = 0; q < 3; ++q)
-        c->A[(size_t)tris[3*t+p]*n + tris[3*t+q]] += w * (G[p]*G[q] + G[3+p]*G[3+q]);
+        c->Lel[(size_t)tris[3*t+p]*n + tris[3*t+q]] += w * (G[p]*G[q] + G[3+p]*G[3+q]);
   }
   for (int hh = 0; hh < H; ++hh) {
     const int32_t *st = c->hinge + 4*hh; const double *K = c->K + 4*hh;
     for (int p = 0; p < 4; ++p)
       for (int q = 0; q < 4; ++q)
-        c->A[(size_t)st[p]*n + st[q]] += c->w_h[hh] * K[p] * K[q];
+        c->Lel[(size_t)st[p]*n + st[q]] += c->w_h[hh] * K[p] * K[q];
   }
+  for (size_t i = 0; i < (size_t)n*n; ++i) c->A[i] = (1.0 + mat->c_beta / h) * c->Lel[i];
+  for (int v = 0; v < n; ++v)
+    c->A[(size_t)v*n+v] += c->mass[v] * (1.0/(h*h) + mat->c_alpha / h) + mat->w_volume;
   if (chol_dense(n, c->A, c->L) != 0) { oracle_destroy(c); return ORACLE_EINVAL; }
   for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) c->LT[(size_t)j*n+i] = c->L[(size_t)i*n+j];
   *out = c;
@@ -447,6 +458,7 @@ void oracle_get_masses(const oracle_cell *c, double *o) { memcpy(o, c->mass, siz
 void oracle_get_areas(const oracle_cell *c, double *o) { memcpy(o, c->area, sizeof(double)*c->T); }
 void oracle_get_G(const oracle_cell *c, double *o) { memcpy(o, c->G, sizeof(double)*6*c->T); }
 void oracle_get_system(const oracle_cell *c, double *o) { memcpy(o, c->A, sizeof(double)*(size_t)c->n*c->n); }
+void oracle_get_elastic_laplacian(const oracle_cell *c, double *o) { memcpy(o, c->Lel, sizeof(double)*(size_t)c->n*c->n); }
 
 /* ---------------------------------------------------------------- the step, piece by piece */
 /* F_t (row-major 3x2):  F^T = G [x_a; x_b; x_c] */
@@ -568,22 +580,50 @@ void oracle_fint(const oracle_cell *c, const double *x, double *f) {
   double *zero = (double*)calloc(3*(size_t)n, sizeof(double));
   oracle_local(c, x, Ps, Pa, Pb, Pv);
   oracle_rhs(c, zero, Ps, Pa, Pb, Pv, f);               /* sum w A^T p */
-  /* minus (sum w A^T A) x = (A_sys - M/h^2) x */
-  double ih2 = 1.0 / (c->h * c->h);
+  /* minus (sum w A^T A) x = (L_el + w_volume I) x */
   for (int i = 0; i < n; ++i)
     for (int d = 0; d < 3; ++d) {
-      double s = 0;
-      for (int j = 0; j < n; ++j) s += c->A[(size_t)i*n+j] * x[3*j+d];
-      s -= c->mass[i] * ih2 * x[3*i+d];
+      double s = m->w_volume * x[3*i+d];
+      for (int j = 0; j < n; ++j) s += c->Lel[(size_t)i*n+j] * x[3*j+d];
       f[3*i+d] -= s;
     }
   (void)m;
   free(Ps); free(Pa); free(Pb); free(Pv); free(zero);
 }
 
+/* Rayleigh damping, implicit (reading A-20): C = c_alpha M + c_beta L_el, f_d = -C (x - x_n)/h.
+ * b += (C/h) x_n  (the other half, (C/h) x, sits in A_sys). */
+void oracle_damping_rhs(const oracle_cell *c, const double *xn, double *b) {
+  int n = c->n; double ca = c->mat.c_alpha / c->h, cb = c->mat.c_beta / c->h;
+  if (ca == 0.0 && cb == 0.0) return;
+  for (int i = 0; i < n; ++i)
+    for (int d = 0; d < 3; ++d) {
+      double s = ca * c->mass[i] * xn[3*i+d];
+      if (cb != 0.0) {
+        double l = 0;
+        for (int j = 0; j < n; ++j) l += c->Lel[(size_t)i*n+j] * xn[3*j+d];
+        s += cb * l;
+      }
+      b[3*i+d] += s;
+    }
+}
+/* dissipation potential of the step, 1/(2h) (x - x_n)^T C (x - x_n): the term the damping adds to
+ * the implicit-Euler objective (its gradient is C (x - x_n)/h = -f_d) */
+double oracle_dissipation(const oracle_cell *c, const double *x, const double *xn) {
+  int n = c->n; double ca = c->mat.c_alpha, cb = c->mat.c_beta, e = 0;
+  if (ca == 0.0 && cb == 0.0) return 0.0;
+  for (int d = 0; d < 3; ++d)
+    for (int i = 0; i < n; ++i) {
+      double ui = x[3*i+d] - xn[3*i+d], l = 0;
+      if (cb != 0.0) for (int j = 0; j < n; ++j) l += c->Lel[(size_t)i*n+j] * (x[3*j+d] - xn[3*j+d]);
+      e += ui * (ca * c->mass[i] * ui + cb * l);
+    }
+  return 0.5 * e / c->h;
+}
+
 /* One time step of ONE cell (SURVEY.md 8(c) "Step"):
  *   s = x_n + h v_n + h^2 f/m;  x^0 = s;
- *   repeat n_iters: local projections at x^k, b, x^{k+1} = A_sys^-1 b;
+ *   repeat n_iters: local projections at x^k, b (+ (C/h) x_n with damping, A-20), x^{k+1} = A_sys^-1 b;
  *   x_{n+1} = x^{n_iters};  v_{n+1} = (x_{n+1} - x_n)/h.
  * Optional outputs: iterates [(n_iters+1)][n][3] (x^0 ... x^{n_iters}) and
  * energies [2*n_iters]: E(x^k;p^k) after each local step, E(x^{k+1};p^k) after each global step. */
@@ -601,10 +641,11 @@ void oracle_step_cell(const oracle_cell *c, double *pos, double *vel, const doub
   if (iterates) memcpy(iterates, x, sizeof(double)*m3);
   for (int k = 0; k < n_iters; ++k) {
     oracle_local(c, x, Ps, Pa, Pb, Pv);
-    if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL);
+    if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos);
     oracle_rhs(c, s, Ps, Pa, Pb, Pv, b);
+    oracle_damping_rhs(c, pos, b);
     oracle_solve(c, b, x);
-    if (energies) energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL);
+    if (energies) energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos);
     if (iterates) memcpy(iterates + (size_t)(k+1)*m3, x, sizeof(double)*m3);
   }
   for (size_t i = 0; i < m3; ++i) { vel[i] = (x[i] - pos[i]) / h; pos[i] = x[i]; }

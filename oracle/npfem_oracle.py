@@ -43,7 +43,7 @@ def lib():
         for name in ("oracle_get_hinges",):
             getattr(L, name).argtypes = [C.c_void_p, _ip]
         for name in ("oracle_get_K", "oracle_get_masses", "oracle_get_areas", "oracle_get_G",
-                     "oracle_get_system"):
+                     "oracle_get_system", "oracle_get_elastic_laplacian"):
             getattr(L, name).argtypes = [C.c_void_p, _dp]
         L.oracle_get_hinge_weights.argtypes = [C.c_void_p, _dp, _dp]
         L.oracle_svd32.argtypes = [_dp, _dp, _dp, _dp]
@@ -65,6 +65,9 @@ def lib():
         L.oracle_energy.restype = C.c_double
         L.oracle_energy.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
         L.oracle_fint.argtypes = [C.c_void_p, _dp, _dp]
+        L.oracle_damping_rhs.argtypes = [C.c_void_p, _dp, _dp]
+        L.oracle_dissipation.restype = C.c_double
+        L.oracle_dissipation.argtypes = [C.c_void_p, _dp, _dp]
         L.oracle_step_cell.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_int, _dp, _dp]
         L.oracle_step.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int]
         L.oracle_num_threads.restype = C.c_int
@@ -196,6 +199,10 @@ class OracleCell:
     def system_matrix(self):
         o = np.empty((self.n, self.n)); lib().oracle_get_system(self._h, _d(o)); return o
 
+    def elastic_laplacian(self):
+        """L_el = sum_t (w_s+w_a) G^T G + sum_h w_h K^T K (the stiffness the c_beta damping uses)."""
+        o = np.empty((self.n, self.n)); lib().oracle_get_elastic_laplacian(self._h, _d(o)); return o
+
     # ---- pieces of the step
     def deformation_gradient(self, t, x):
         x = _f64(x); F = np.empty((3, 2))
@@ -227,6 +234,15 @@ class OracleCell:
     def fint(self, x):
         x = _f64(x); f = np.empty((self.n, 3))
         lib().oracle_fint(self._h, _d(x), _d(f)); return f
+
+    def damping_rhs(self, xn):
+        """(C/h) x_n with C = c_alpha M + c_beta L_el: what the damping adds to the rhs (A-20)."""
+        xn = _f64(xn); b = np.zeros((self.n, 3))
+        lib().oracle_damping_rhs(self._h, _d(xn), _d(b)); return b
+
+    def dissipation(self, x, xn):
+        x, xn = _f64(x), _f64(xn)
+        return float(lib().oracle_dissipation(self._h, _d(x), _d(xn)))
 
     # ---- whole steps
     def step_cell(self, pos, vel, fext, n_iters, trace=False):

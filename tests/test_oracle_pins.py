@@ -320,7 +320,7 @@ def test_create_rejects_bad_meshes():
     with pytest.raises(ValueError):
         O.OracleCell(tris[:, [0, 2, 1]], rest, mat, DT)           # inside-out: V0 <= 0
     with pytest.raises(ValueError):
-        O.OracleCell(tris, rest, dict(mat, c_alpha=0.1), DT)      # damping not on the hot path (A-5)
+        O.OracleCell(tris, rest, dict(mat, c_alpha=-0.1), DT)     # negative damping
     with pytest.raises(ValueError):
         O.OracleCell(tris, rest, dict(mat, s_min=1.2, s_max=1.0), DT)
 
@@ -475,3 +475,105 @@ def test_oracle_reproduces_its_committed_config1_result():
     scale = np.abs(ref[:, :3]).max()
     assert np.abs(disp - ref[:, :3]).max() <= 1e-9 * scale      # fp64 summation-order slack
     assert np.abs(vel[0] - ref[:, 3:]).max() <= 1e-9 * np.abs(ref[:, 3:]).max()
+
+
+# ----------------------------------------------------------------------------- damping (A-20)
+def test_P13_free_cell_with_mass_proportional_damping_decays_at_the_implicit_euler_rate():
+    """No elasticity, c_alpha > 0: M (v' - v)/h = f - c_alpha M v'  =>  v' = r (v + h f/m),
+    r = 1/(1 + h c_alpha).  After N steps (geometric series):
+        v_N = r^N v_0 + (h f/m) r (1 - r^N)/(1 - r),   x_N = x_0 + h sum_{k=1..N} v_k."""
+    rest, tris = W.rest_shape("plt", 1)
+    ca = 0.7
+    mat = W.default_material(rest, tris, k_strain=0, k_area=0, k_bend=0, w_volume=0, c_alpha=ca)
+    c = O.OracleCell(tris, rest, mat, DT)
+    rng = np.random.default_rng(31)
+    f = 1e-3 * rng.standard_normal(rest.shape)
+    v0 = 1e-2 * rng.standard_normal(rest.shape)
+    a = DT * f / c.masses()[:, None]
+    r = 1.0 / (1.0 + DT * ca)
+    x, v = rest.copy(), v0.copy()
+    N = 9
+    for _ in range(N):
+        x, v = c.step_cell(x, v, f, 2)
+    vN = r ** N * v0 + a * r * (1 - r ** N) / (1 - r)
+    # sum_{k=1..N} v_k with v_k = r^k v0 + a r (1 - r^k)/(1 - r)
+    geo = r * (1 - r ** N) / (1 - r)
+    xN = rest + DT * (geo * v0 + a * r / (1 - r) * (N - geo))
+    assert np.abs(v - vN).max() < 1e-12 and np.abs(x - xN).max() < 1e-13   # v = (x' - x)/h: rounding / h
+    assert np.abs(vN).max() < np.abs(v0 + N * a).max()              # and it does damp
+
+
+def test_P14_stiffness_proportional_damping_leaves_rigid_translation_alone():
+    """L_el has zero row sums (it only sees differences), so c_beta does not act on a uniform
+    velocity: the rest shape drifting at constant velocity stays rigid and keeps its velocity."""
+    c, rest, _, _ = make_cell("rbc", 2, c_beta=0.5)
+    L = c.elastic_laplacian()
+    assert np.abs(L - L.T).max() < 1e-12 and np.abs(L.sum(axis=1)).max() < 1e-10
+    assert np.linalg.eigvalsh(L).min() > -1e-10
+    v0 = np.tile(np.array([3e-3, -1e-3, 2e-3]), (rest.shape[0], 1))
+    x, v = rest.copy(), v0.copy()
+    for _ in range(5):
+        x, v = c.step_cell(x, v, np.zeros_like(rest), 4)
+    assert np.abs(x - (rest + 5 * DT * v0)).max() < 1e-12 and np.abs(v - v0).max() < 1e-11
+    # while a deformation rate IS damped: stretch velocity field, compare against c_beta = 0
+    c0, _, _, _ = make_cell("rbc", 2)
+    vs = 1e-2 * np.random.default_rng(34).standard_normal(rest.shape)     # vertex-wise noise: all deformation
+    _, v_damped = c.step_cell(rest, vs, np.zeros_like(rest), 20)
+    _, v_free = c0.step_cell(rest, vs, np.zeros_like(rest), 20)
+    assert np.linalg.norm(v_damped) < 0.9 * np.linalg.norm(v_free)
+
+
+def test_P15_damped_global_update_is_quasi_newton_step_on_the_damped_objective():
+    """g(x) = 1/2 ||x-s||^2_M/h^2 + E_el(x) + 1/(2h) (x-x_n)^T C (x-x_n), C = c_alpha M + c_beta L_el;
+    one sweep = x - A_sys^-1 grad g(x), with A_sys = (1/h^2 + c_alpha/h) M + (1 + c_beta/h) L_el + w_vol I.
+    C is rebuilt here from the masses and the elastic Laplacian; the dissipation term is checked
+    against its own finite differences."""
+    c, rest, _, mat = make_cell("rbc", 2, c_alpha=0.3, c_beta=0.05)
+    rng = np.random.default_rng(32)
+    xn = rest + 0.01 * rng.standard_normal(rest.shape)
+    vn = 1e-2 * rng.standard_normal(rest.shape)
+    f = 5e-3 * rng.standard_normal(rest.shape)
+    m = c.masses()[:, None]
+    Cmat = 0.3 * np.diag(c.masses()) + 0.05 * c.elastic_laplacian()
+    A = c.system_matrix()
+    A_expect = np.diag(c.masses()) / DT ** 2 + c.elastic_laplacian() + mat["w_volume"] * np.eye(rest.shape[0]) + Cmat / DT
+    assert np.abs(A - A_expect).max() < 1e-10 * np.abs(A).max()
+    _, _, its, en = c.step_cell(xn, vn, f, 4, trace=True)
+    s = its[0]
+    assert np.abs(s - (xn + DT * vn + DT ** 2 * f / m)).max() < 1e-14
+    for k in range(4):
+        grad = m * (its[k] - s) / DT ** 2 - c.fint(its[k]) + Cmat @ (its[k] - xn) / DT
+        pred = its[k] - c.solve(grad)
+        assert np.abs(pred - its[k + 1]).max() < 1e-12
+    assert (np.diff(en) <= 1e-12 * np.abs(en[:-1])).all()            # damped objective is monotone too
+    # dissipation potential: value and gradient
+    x = its[2]
+    assert c.dissipation(x, xn) == pytest.approx(0.5 * np.sum((x - xn) * (Cmat @ (x - xn))) / DT, rel=1e-12)
+    eps = 1e-6
+    e = np.zeros_like(x); e[5, 1] = eps
+    fd = (c.dissipation(x + e, xn) - c.dissipation(x - e, xn)) / (2 * eps)
+    assert fd == pytest.approx((Cmat @ (x - xn) / DT)[5, 1], rel=1e-6)
+    assert np.abs(c.damping_rhs(xn) - Cmat @ xn / DT).max() < 1e-12 * np.abs(Cmat @ xn / DT).max()
+
+
+def test_P16_damping_dissipates_mechanical_energy():
+    """Free vibration from a stretched state: kinetic + elastic energy after 30 steps is lower
+    with viscoelastic damping than without, for c_alpha alone, c_beta alone and both."""
+    rest, tris = W.rest_shape("rbc", 2)
+    z = np.zeros_like(rest)
+
+    def mech_energy(cell, x, v):
+        proj = cell.local(x)
+        _, parts = cell.energy(x, x, proj, parts=True)               # s = x: no inertial term
+        return 0.5 * np.sum(cell.masses()[:, None] * v * v) + parts[1:].sum()
+
+    out = {}
+    for key, over in (("none", {}), ("alpha", dict(c_alpha=0.5)), ("beta", dict(c_beta=0.05)),
+                      ("both", dict(c_alpha=0.5, c_beta=0.05))):
+        cell = O.OracleCell(tris, rest, W.default_material(rest, tris, **over), DT)
+        x, v = rest * 1.05, z.copy()
+        for _ in range(30):
+            x, v = cell.step_cell(x, v, z, 10)
+        out[key] = mech_energy(cell, x, v)
+    assert out["alpha"] < out["none"] and out["beta"] < out["none"]
+    assert out["both"] < min(out["alpha"], out["beta"])
