@@ -39,10 +39,11 @@ extern "C" {
 
 #define NPFEM_OK 0
 #define NPFEM_EINVAL (-1) /* bad argument, non-closed / inconsistently oriented mesh, V0 <= 0,    */
-                          /* degenerate rest triangle, band with min > max, damping != 0          */
+                          /* degenerate rest triangle, band with min > max, negative damping      */
 #define NPFEM_ENOMEM (-2) /* host allocation failed                                               */
 #define NPFEM_ECUDA (-3)  /* a CUDA call failed (message holds the CUDA error string)             */
-#define NPFEM_ELIMIT (-4) /* mesh larger than one CTA can hold (n_verts > 1024 or shared memory)  */
+#define NPFEM_ELIMIT (-4) /* mesh larger than one CTA can hold (n_verts > 1024 or shared memory;   */
+                          /* with damping: more than 768 threads per cell)                         */
 
 typedef struct npfem_handle_s* npfem_handle; /* opaque; one per cell TYPE */
 typedef struct npfem_plan_s* npfem_plan;     /* opaque; host-only create-time data (no CUDA)      */
@@ -54,7 +55,10 @@ typedef struct {
   double k_area, a_min, a_max;   /* triangle area weight per rest area; band on sigma1*sigma2       */
   double k_bend;                 /* hinge weight, multiplies 3/(A0+A1)                              */
   double w_volume, v_min, v_max; /* per-cell volume weight; band on V/V0                            */
-  double c_alpha, c_beta;        /* damping (PAPER.md:145,183 Calpha/Cbeta); must be 0 (A-5)        */
+  double c_alpha, c_beta;        /* viscoelastic damping (PAPER.md:60, :145, :183 Calpha / Cbeta),   */
+                                 /* >= 0: implicit Rayleigh damping f_d = -(c_alpha M + c_beta L_el) */
+                                 /* v_{n+1}, L_el = the strain + area + bending stiffness (A-20);    */
+                                 /* c_alpha in 1/time, c_beta in time                                */
 } npfem_material;
 
 /* Tuning knobs that do not change what is computed beyond fp32 rounding.  Pass NULL for defaults. */
@@ -108,7 +112,8 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
  *   n_iters   >= 0 (0 = pure inertial prediction)
  *   cuda_stream  a cudaStream_t (NULL = default stream); the call only enqueues work
  * Result: x_{n+1} = x_n + inc, v_{n+1} = inc/h with inc = h v_n + h^2 f/m + d, d the projective-
- * dynamics correction after n_iters iterations.  Errors: NPFEM_EINVAL,
+ * dynamics correction after n_iters iterations; with c_alpha, c_beta != 0 the
+ * iterations minimise the damped implicit-Euler objective (A-20).  Errors: NPFEM_EINVAL,
  * NPFEM_ECUDA (launch failure).
  */
 int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,

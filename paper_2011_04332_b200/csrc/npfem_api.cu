@@ -242,11 +242,12 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   //   0: packed byte offsets 16*id of (a,b) (c,d) (f1,f2) (f3,f4)   1: t1 i00 i01 i11 w_s
   //   2: t2 i00 i01 i11 w_s      3: t1 w_a, t2 w_a, he, 0           4..8: hinge e: Kp Kq Ko r'
   std::vector<uint32_t> elem_c((size_t)kElemGroups * E * 4, 0u);
-  std::vector<float> h2m(NP, 0.0f), mh2(NP, 0.0f);
+  std::vector<float> h2m(NP, 0.0f), mh2(NP, 0.0f), dmp(NP, 0.0f);
   for (int i = 0; i < n; ++i) {
     perm16[i] = (uint16_t)P.perm[i];
     h2m[i] = P.h2_over_m[i];
     mh2[i] = P.m_over_h2[i];
+    dmp[i] = P.damp_m[i];
   }
   auto fbits = [](float x) { uint32_t u; std::memcpy(&u, &x, 4); return u; };
   for (int e = 0; e < E; ++e) {
@@ -283,6 +284,7 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
       {P.inc_off.data(), P.inc_off.size() * 2, 0},    {P.ring_ptr.data(), P.ring_ptr.size() * 2, 0},
       {P.ring_off.data(), P.ring_off.size() * 2, 0},  {P.blk_ptr.data(), P.blk_ptr.size() * 4, 0},
       {P.blk_col.data(), P.blk_col.size() * 2, 0},    {P.blk_val.data(), P.blk_val.size() * 4, 0},
+      {dmp.data(), dmp.size() * 4, 0},
   };
   size_t total = 0;
   for (auto& sct : secs) { sct.off = total; total += align_up(sct.bytes, 256); }
@@ -313,6 +315,9 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.blk_ptr = reinterpret_cast<const int*>(base + secs[9].off);
   D.blk_col = reinterpret_cast<const uint16_t*>(base + secs[10].off);
   D.blk_val = reinterpret_cast<const float*>(base + secs[11].off);
+  D.damp_m = reinterpret_cast<const float*>(base + secs[12].off);
+  D.cbh = (float)(P.mat.c_beta / P.h);
+  D.damped = P.damped ? 1 : 0;
   D.L = smem_layout(n, E, P.nvb, P.cells_per_cta);
   if (max_cells > 0) {   // everything any later step entry point needs exists now
     rc = create_pipeline(H, max_cells);

@@ -62,7 +62,9 @@ struct Plan {
   std::vector<ElemConst> elem;       // [E]
   std::vector<int32_t> elem_tris;    // [E][2] caller triangle ids (second = -1 for a single)
   std::vector<float> h2_over_m;      // [n]
-  std::vector<float> m_over_h2;      // [n]
+  std::vector<float> m_over_h2;      // [n] m (1/h^2 + c_alpha/h)
+  std::vector<float> damp_m;         // [n] m c_alpha/h
+  bool damped = false;               // c_alpha != 0 or c_beta != 0 (reading A-20)
   std::vector<uint16_t> inc_ptr;     // [n+1] CSR over the element slots a vertex gathers from
   std::vector<uint16_t> inc_off;     // byte offset of the slot's float4 in the out buffer
   std::vector<uint16_t> ring_ptr;    // [n+1] CSR over the cyclically ordered ring neighbours

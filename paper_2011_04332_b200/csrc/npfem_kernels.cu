@@ -136,8 +136,20 @@ __device__ __forceinline__ float hyperbola_p(float s1, float s2, float q, float 
 //   - triangle strain   w_s ||F - P_s||^2/2,  P_s = U clamp(Sigma,[s_min,s_max]) V^T
 //   - triangle area     w_a ||F - P_a||^2/2,  P_a = U Sigma' V^T, sigma1' sigma2' = clamp(sigma1 sigma2)
 // on vertices 1 and 2 (vertex 0 receives -(f1 + f2)).  SURVEY.md 8(c) step 2.
+// KIND 1 (damped, reading A-20): the stiffness-proportional damping adds -(c_beta/h)(w_s + w_a) G^T F,
+// i.e. a shift of both g_i.  KIND 2: the linear operator alone, +(c_beta/h)(w_s + w_a) G^T F (used
+// once per step on y = x_n - c to form the constant part of the damping force).
+template <int KIND>
 __device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, float i11, float ws,
                                          float wa, const DevParams& P, F3& f1, F3& f2) {
+  if (KIND == 2) {
+    const float coef = P.cbh * (ws + wa);
+    const F3 Q0 = (coef * i00) * e1;
+    const F3 Q1 = coef * fma3(i01, e1, i11 * e2);
+    f1 = fma3(i00, Q0, i01 * Q1);
+    f2 = i11 * Q1;
+    return;
+  }
   const F3 F0 = i00 * e1;
   const F3 F1 = fma3(i01, e1, i11 * e2);
   const float C11 = dot(F0, F0), C12 = dot(F0, F1), C22 = dot(F1, F1);
@@ -160,6 +172,10 @@ __device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, flo
     g1 = fmaf(wa, fmaf(q, p, -s1) * r1, g1);
     g2 = fmaf(wa, fmaf(q, frcp(p), -s2) * r2, g2);
   }
+  if (KIND == 1) {
+    const float shift = P.cbh * (ws + wa);
+    g1 -= shift; g2 -= shift;
+  }
   const float gbar = 0.5f * (g1 + g2);
   const float rho = (g1 - g2) * frcp(fmaxf(Delta, 1e-30f));
   const float S00 = fmaf(rho, 0.5f * dC, gbar), S11 = fmaf(-rho, 0.5f * dC, gbar), S01 = rho * C12;
@@ -172,10 +188,15 @@ __device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, flo
 // Bending hinge on the edge (p,q) with own opposite vertex o and the vertex f across:
 // kv = sum K_i z_i written with edges from p (rows of K sum to 0), scaled so that adding
 // K_i * kv to vertex i applies the residual  w_h K_i (r_h k/|k| - k)  (bending).
-__device__ __forceinline__ F3 hinge_vec(float Kq, float Ko, float Kf, float rp, F3 epq, F3 epo, F3 epf) {
+// KIND 1: with the damping term -(c_beta/h) w_h K_i k the factor becomes r/|k| - 1 - c_beta/h;
+// KIND 2: the linear operator alone, factor +c_beta/h.
+template <int KIND>
+__device__ __forceinline__ F3 hinge_vec(float Kq, float Ko, float Kf, float rp, F3 epq, F3 epo, F3 epf,
+                                        float cbh) {
   const F3 kv = fma3(Kq, epq, fma3(Ko, epo, Kf * epf));
+  if (KIND == 2) return cbh * kv;
   const float nk2 = fmaxf(dot(kv, kv), 1e-30f);
-  const float cf = fmaf(rp, frsqrt(nk2), -1.0f);
+  const float cf = fmaf(rp, frsqrt(nk2), KIND == 1 ? -1.0f - cbh : -1.0f);
   return cf * kv;
 }
 
@@ -222,6 +243,7 @@ __device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
 // Local step of one element for one cell: membrane residuals of its two triangles and the five
 // hinges it sees, summed per own vertex (a,b,c,d) into out4[slot * E].  ec = the element's
 // constants in shared memory (group g at ec[g * E], npfem_api.cu), zc = the cell's z4 array.
+template <int KIND>
 __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, int E,
                                                  const unsigned char* __restrict__ zc,
                                                  const DevParams& P, float4* __restrict__ out4) {
@@ -240,7 +262,7 @@ __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, 
     const float4 hk = ec[4 * E];
     const float Kp = hk.x, Kq = hk.y, Ko = hk.z;
     const float Kf = -(Kp + Kq + Ko), he = m3.z, hf = fmaf(2.0f, he, -1.0f);
-    const F3 kv = hinge_vec(Kq, Ko, Kf, hk.w, eab, eac, ead);
+    const F3 kv = hinge_vec<KIND>(Kq, Ko, Kf, hk.w, eab, eac, ead, P.cbh);
     fa = fma3(he * Kp, kv, fa); fb = fma3(he * Kq, kv, fb);
     fc = fma3(Ko, kv, fc);      fd = fma3(hf * Kf, kv, fd);
   }
@@ -248,27 +270,27 @@ __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, 
   {   // (b,c | a ; f1)
     const float4 hk = ec[5 * E];
     const F3 zf = lds3(zc, id_f12 & 0xffffu);
-    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, ebc, eba, zf - zb);
+    const F3 kv = hinge_vec<KIND>(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, ebc, eba, zf - zb, P.cbh);
     fb = fma3(0.5f * hk.x, kv, fb); fc = fma3(0.5f * hk.y, kv, fc); fa = fma3(hk.z, kv, fa);
   }
   {   // (c,a | b ; f2)
     const float4 hk = ec[6 * E];
     const F3 zf = lds3(zc, id_f12 >> 16);
     const F3 eca = {-eac.x, -eac.y, -eac.z}, ecb = {-ebc.x, -ebc.y, -ebc.z};
-    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, eca, ecb, zf - zc3);
+    const F3 kv = hinge_vec<KIND>(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, eca, ecb, zf - zc3, P.cbh);
     fc = fma3(0.5f * hk.x, kv, fc); fa = fma3(0.5f * hk.y, kv, fa); fb = fma3(hk.z, kv, fb);
   }
   {   // (a,d | b ; f3)
     const float4 hk = ec[7 * E];
     const F3 zf = lds3(zc, id_f34 & 0xffffu);
-    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, ead, eab, zf - za);
+    const F3 kv = hinge_vec<KIND>(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, ead, eab, zf - za, P.cbh);
     fa = fma3(0.5f * hk.x, kv, fa); fd = fma3(0.5f * hk.y, kv, fd); fb = fma3(hk.z, kv, fb);
   }
   {   // (d,b | a ; f4)
     const float4 hk = ec[8 * E];
     const F3 zf = lds3(zc, id_f34 >> 16);
     const F3 edb = {-ebd.x, -ebd.y, -ebd.z}, eda = {-ead.x, -ead.y, -ead.z};
-    const F3 kv = hinge_vec(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, edb, eda, zf - zd);
+    const F3 kv = hinge_vec<KIND>(hk.y, hk.z, -(hk.x + hk.y + hk.z), hk.w, edb, eda, zf - zd, P.cbh);
     fd = fma3(0.5f * hk.x, kv, fd); fb = fma3(0.5f * hk.y, kv, fb); fa = fma3(hk.z, kv, fa);
   }
   // ---- membranes, last (the hinge pass is over, few values are live): t1 = (a,b,c) from a;
@@ -276,8 +298,8 @@ __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, 
   {
     const float4 m1 = ec[E], m2 = ec[2 * E];
     F3 t1b, t1c, t2a, t2d;
-    membrane(eab, eac, m1.x, m1.y, m1.z, m1.w, m3.x, P, t1b, t1c);
-    membrane(eba, ebd, m2.x, m2.y, m2.z, m2.w, m3.y, P, t2a, t2d);
+    membrane<KIND>(eab, eac, m1.x, m1.y, m1.z, m1.w, m3.x, P, t1b, t1c);
+    membrane<KIND>(eba, ebd, m2.x, m2.y, m2.z, m2.w, m3.y, P, t2a, t2d);
     fa = fa + (t2a - (t1b + t1c));
     fb = fb + (t1b - (t2a + t2d));
     fc = fc + t1c;
@@ -384,7 +406,7 @@ __device__ __forceinline__ void block_run(float (&acc)[4], float (&accx)[4], con
 // The fused step kernel.  MODE 1: global step with fp32 FMAs (comparison path); MODE 2: 3xTF32
 // mma.sync on the block-sparse inverse.
 // ------------------------------------------------------------------------------------------
-template <int MODE, int MAXT>
+template <int MODE, int MAXT, bool DAMP>
 __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   unsigned char* const z4b = smem_raw + P.L.z4;                        // [k][NP] float4 iterate z
@@ -402,9 +424,11 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const int kact = min(P.k, P.n_cells - cell0);
   const int cellz = NP * 16;                      // bytes of one cell's z4
 
-  // ---- tensor memory: 64 columns per group of 4 warps (s: 0..14, d: 16..30, rhs: 32..47, u0: 48..62)
+  // ---- tensor memory: 64 columns per group of 4 warps (s: 0..14, d: 16..30, rhs: 32..47, u0: 48..62);
+  //      with damping 16 more (64..78: the part of the damping force that is constant over a step)
+  constexpr uint32_t kTmemGroup = DAMP ? 80u : 64u;
   uint32_t tmem_cols = 64;
-  while (tmem_cols < 64u * ((nwarps + 3) >> 2)) tmem_cols <<= 1;
+  while (tmem_cols < kTmemGroup * ((nwarps + 3) >> 2)) tmem_cols <<= 1;
   if (warp == 0) {
     const uint32_t sa = (uint32_t)__cvta_generic_to_shared(&tmem_base_s);
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(sa), "r"(tmem_cols) : "memory");
@@ -429,7 +453,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const uint32_t ta = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 64);
+  const uint32_t ta = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * kTmemGroup);
 
   // ---- prologue: stage each cell's pos / vel / fext rows through shared memory with coalesced
   //      loads, hand every vertex to its owner thread, centroid, local coordinates, prediction
@@ -483,6 +507,52 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     tmem_st16(ta + 32, zero16);
     tmem_st16(ta + 48, ur);
     __syncthreads();
+    if (DAMP) {
+      // Rayleigh damping, implicit (reading A-20): the damping force -(C/h)(x - x_n),
+      // C = c_alpha M + c_beta L_el, with x - x_n = u0 + d and L_el (u0 + d) = L_el z - L_el y:
+      //   -(c_alpha/h) m d      -> folded into the diagonal m (1/h^2 + c_alpha/h) of the residual
+      //   -(c_beta/h) L_el z    -> folded into the element pass (a shift of the membrane factors and
+      //                            of the hinge factor)
+      //   Q = (c_beta/h) L_el y - (c_alpha/h) m u0   -> constant over the step: formed here, once,
+      //                            by one pass of the linear operator over y, and parked in TMEM.
+      float qreg[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) qreg[i] = 0.f;
+      const float dm = P.damp_m[v];
+      if (P.cbh != 0.0f) {
+        const uint4 vr0q = P.vrole[2 * v];
+        const int icnt = vr0q.w & 0xff;
+#pragma unroll
+        for (int c = 0; c < kMaxCellsPerCta; ++c) {
+          if (c < kact) {
+            float4* z4c = reinterpret_cast<float4*>(z4b) + c * NP;
+            if (isv) z4c[v] = make_float4(sreg[3 * c] - ur[3 * c], sreg[3 * c + 1] - ur[3 * c + 1],
+                                          sreg[3 * c + 2] - ur[3 * c + 2], 0.f);        // y = s - u0
+            __syncthreads();
+            if (tid < E)
+              element_residual<2>(ecs + tid, E, z4b + c * cellz, P, reinterpret_cast<float4*>(rbb) + tid);
+            __syncthreads();
+            if (isv) {
+              F3 q = {0.f, 0.f, 0.f};
+              const uint32_t ioff[kRegList / 2] = {vr0q.x, vr0q.y, vr0q.z};
+#pragma unroll
+              for (int i = 0; i < kRegList; ++i)
+                if (i < icnt) q = q + lds3(rbb, (i & 1) ? (ioff[i >> 1] >> 16) : (ioff[i >> 1] & 0xffffu));
+              if (icnt > kRegList) {
+                const uint16_t* inc_tail = P.inc_off + P.inc_ptr[v];
+                for (int i = kRegList; i < icnt; ++i) q = q + lds3(rbb, inc_tail[i]);
+              }
+              qreg[3 * c] = q.x; qreg[3 * c + 1] = q.y; qreg[3 * c + 2] = q.z;
+              z4c[v] = make_float4(sreg[3 * c], sreg[3 * c + 1], sreg[3 * c + 2], 0.f);   // back to z = s
+            }
+            __syncthreads();
+          }
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < 15; ++i) qreg[i] = fmaf(-dm, ur[i], qreg[i]);
+      tmem_st16(ta + 64, qreg);
+    }
   }
 
   // ---- iterations
@@ -507,7 +577,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     // so the vertex phase of cell c and the element pass of cell c+1 share one barrier interval
     auto elements_and_gradient = [&](int cc) {
       const unsigned char* zcc = z4b + cc * cellz;
-      if (is_e) element_residual(ec_t, E, zcc, P, reinterpret_cast<float4*>((cc & 1) ? rab : rbb) + tid);
+      if (is_e) element_residual<DAMP ? 1 : 0>(ec_t, E, zcc, P, reinterpret_cast<float4*>((cc & 1) ? rab : rbb) + tid);
       vr0 = P.vrole[2 * v];
       if (use_vol) {
         float S1 = 0.f, S2 = 0.f;
@@ -608,6 +678,11 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     {
       float ee[16], dd[16];
       tmem_ld16(ta + 32, ee);
+      if (DAMP) {
+        tmem_ld16(ta + 64, dd);
+#pragma unroll
+        for (int m = 0; m < 15; ++m) ee[m] += dd[m];
+      }
       tmem_ld16(ta + 16, dd);
       const float nmh2 = -__uint_as_float(P.vrole[2 * v + 1].w);
       if (isvp) {
@@ -738,11 +813,12 @@ cudaError_t configure_kernels(int smem_bytes) {
   cudaError_t e;
   (void)smem_bytes;
   smem_bytes = kSmemMaxDynamic;   // opt in once to the largest carve-out any cell type may need
-#define NPFEM_CFG(MODE, MAXT)                                                                   \
-  e = cudaFuncSetAttribute(npfem_step_kernel<MODE, MAXT>,                                       \
+#define NPFEM_CFG(MODE, MAXT, DAMP)                                                             \
+  e = cudaFuncSetAttribute(npfem_step_kernel<MODE, MAXT, DAMP>,                                 \
                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);            \
   if (e != cudaSuccess) return e;
-  NPFEM_CFG(1, 672) NPFEM_CFG(1, 1024) NPFEM_CFG(2, 672) NPFEM_CFG(2, 1024)
+  NPFEM_CFG(1, 672, false) NPFEM_CFG(1, 1024, false) NPFEM_CFG(2, 672, false) NPFEM_CFG(2, 1024, false)
+  NPFEM_CFG(1, 672, true) NPFEM_CFG(1, 1024, true) NPFEM_CFG(2, 672, true) NPFEM_CFG(2, 1024, true)
 #undef NPFEM_CFG
   return cudaSuccess;
 }
@@ -751,13 +827,17 @@ cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mod
                         cudaStream_t stream) {
   if (p.n_cells <= 0) return cudaSuccess;
   const int grid = (p.n_cells + p.k - 1) / p.k;
+#define NPFEM_LAUNCH(MODE, MAXT)                                                                \
+  do {                                                                                          \
+    if (p.damped) npfem_step_kernel<MODE, MAXT, true><<<grid, threads, smem_bytes, stream>>>(p); \
+    else npfem_step_kernel<MODE, MAXT, false><<<grid, threads, smem_bytes, stream>>>(p);        \
+  } while (0)
   if (threads <= 672) {
-    if (mode == 2) npfem_step_kernel<2, 672><<<grid, threads, smem_bytes, stream>>>(p);
-    else npfem_step_kernel<1, 672><<<grid, threads, smem_bytes, stream>>>(p);
+    if (mode == 2) NPFEM_LAUNCH(2, 672); else NPFEM_LAUNCH(1, 672);
   } else {
-    if (mode == 2) npfem_step_kernel<2, 1024><<<grid, threads, smem_bytes, stream>>>(p);
-    else npfem_step_kernel<1, 1024><<<grid, threads, smem_bytes, stream>>>(p);
+    if (mode == 2) NPFEM_LAUNCH(2, 1024); else NPFEM_LAUNCH(1, 1024);
   }
+#undef NPFEM_LAUNCH
   return cudaGetLastError();
 }
 

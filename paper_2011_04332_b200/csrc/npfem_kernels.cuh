@@ -19,10 +19,13 @@ struct DevParams {
   int n, E, nvb, k, n_cells, cell_stride, n_iters, vol_iters;
   float h, w_volume, V0, Vmin, Vmax;       // Vmin/Vmax = v_min*V0, v_max*V0
   float s_min, s_max, a_min, a_max;
+  float cbh;                               // c_beta / h (stiffness-proportional damping, A-20)
+  int damped;                              // c_alpha != 0 or c_beta != 0
   const uint16_t* perm;                    // [NP] internal -> caller vertex (padding: 0)
   const float4* elem_c;                    // [kElemGroups][E] element constants (npfem_api.cu)
   const float* h2_over_m;                  // [NP]
-  const float* m_over_h2;                  // [NP]
+  const float* m_over_h2;                  // [NP] m (1/h^2 + c_alpha/h)
+  const float* damp_m;                     // [NP] m c_alpha / h
   const uint4* vrole;                      // [NP][2] vertex-role constants (npfem_api.cu)
   const uint16_t* inc_ptr;                 // [n+1]
   const uint16_t* inc_off;                 // byte offsets into the element result buffer

@@ -118,8 +118,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
   if (n > kMaxVerts) return fail(NPFEM_ELIMIT, "n_verts exceeds 1024 (one CTA owns whole cells)");
   if (mat->s_min > mat->s_max || mat->a_min > mat->a_max || mat->v_min > mat->v_max)
     return fail(NPFEM_EINVAL, "clamp band with min > max");
-  if (mat->c_alpha != 0.0 || mat->c_beta != 0.0)
-    return fail(NPFEM_EINVAL, "damping (c_alpha, c_beta) must be 0 on the hot path (DESIGN.md A-5)");
+  if (!(mat->c_alpha >= 0.0) || !(mat->c_beta >= 0.0))
+    return fail(NPFEM_EINVAL, "damping coefficients c_alpha, c_beta must be >= 0 (DESIGN.md A-20)");
   if (!(mat->cell_mass > 0.0)) return fail(NPFEM_EINVAL, "cell_mass must be positive");
   if (mat->k_strain < 0 || mat->k_area < 0 || mat->k_bend < 0 || mat->w_volume < 0)
     return fail(NPFEM_EINVAL, "negative weight");
@@ -236,11 +236,13 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     }
   if (hc != H) return fail(NPFEM_EINVAL, "edge count does not match 3T/2");
 
-  // ---- A_sys (caller order)
+  // ---- A_sys (caller order) = (1/h^2 + c_alpha/h) M + (1 + c_beta/h) L_el + w_volume I, where
+  //      L_el = sum_t (w_s + w_a) G^T G + sum_h w_h K^T K.  c_alpha = c_beta = 0: the undamped
+  //      system; otherwise the implicit Rayleigh damping of reading A-20
   const double ih2 = 1.0 / (dt * dt);
+  const double mass_scale = ih2 + mat->c_alpha / dt, el_scale = 1.0 + mat->c_beta / dt;
   P->A.assign((size_t)n * n, 0.0);
   std::vector<double>& A = P->A;
-  for (int v = 0; v < n; ++v) A[(size_t)v * n + v] = P->mass[v] * ih2 + mat->w_volume;
   for (int t = 0; t < T; ++t) {
     double i00 = P->tri_dminv[3 * t], i01 = P->tri_dminv[3 * t + 1], i11 = P->tri_dminv[3 * t + 2];
     // columns of G = D_m^-T [[-1,1,0],[-1,0,1]]: vertex b -> (i00, i01), c -> (0, i11), a -> -(b + c)
@@ -257,6 +259,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     for (int p = 0; p < 4; ++p)
       for (int q = 0; q < 4; ++q) A[(size_t)hv[p] * n + hv[q]] += wh * K[p] * K[q];
   }
+  for (double& a : A) a *= el_scale;
+  for (int v = 0; v < n; ++v) A[(size_t)v * n + v] += P->mass[v] * mass_scale + mat->w_volume;
 
   // ---- T = A_sys^-1 (fp64): Cholesky A = L L^T, M = L^-1, T = M^T M
   std::vector<double> L((size_t)n * n, 0.0), M((size_t)n * n, 0.0), Tinv((size_t)n * n, 0.0);
@@ -433,11 +437,14 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
   // ---- per-vertex constants (internal numbering)
   P->h2_over_m.resize(n);
   P->m_over_h2.resize(n);
+  P->damp_m.resize(n);
   for (int i = 0; i < n; ++i) {
     double m = P->mass[P->perm[i]];
     P->h2_over_m[i] = (float)(dt * dt / m);
-    P->m_over_h2[i] = (float)(m * ih2);
+    P->m_over_h2[i] = (float)(m * mass_scale);          // inertial + mass-proportional damping diagonal
+    P->damp_m[i] = (float)(m * mat->c_alpha / dt);      // (c_alpha/h) m: acts on the predicted increment
   }
+  P->damped = mat->c_alpha != 0.0 || mat->c_beta != 0.0;
 
   // ---- elements: pair triangles across shared edges (a matching of the dual graph, which is
   //      cubic and bridgeless for a closed manifold, so a perfect matching exists; greedy by
@@ -665,6 +672,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
   int need = std::max(nvb * 8, E);
   P->threads = (need + 31) / 32 * 32;
   if (P->threads > 1024) return fail(NPFEM_ELIMIT, "mesh needs more than 1024 threads per cell");
+  if (P->damped && P->threads > 768)   // 80 tensor-memory columns per 4 warps: 6 groups fit the 512
+    return fail(NPFEM_ELIMIT, "damping needs more tensor-memory columns than a CTA of more than 768 threads has");
   const int smem_max = kSmemMaxDynamic;
   int k = o.cells_per_cta ? o.cells_per_cta : kMaxCellsPerCta;
   while (k > 1 && smem_layout(n, E, nvb, k).total > smem_max) {

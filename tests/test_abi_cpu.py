@@ -153,7 +153,7 @@ def test_argument_errors_are_codes_not_crashes():
     rest, tris = W.rest_shape("rbc", 1)
     mat = W.default_material(rest, tris)
     NpfemPlan(tris, rest, mat, DT)
-    bad = dict(mat, c_alpha=0.1)
+    bad = dict(mat, c_alpha=-0.1)
     with pytest.raises(NpfemError) as e:
         NpfemPlan(tris, rest, bad, DT)
     assert e.value.code == -1 and "damping" in str(e.value)
@@ -183,3 +183,20 @@ def test_no_cpu_fallback_create_fails_loudly_without_cuda():
     with pytest.raises(NpfemError) as e:
         NpfemHandle(tris, rest, W.default_material(rest, tris), DT)
     assert e.value.code == -3
+
+
+def test_damped_system_matrix_matches_the_oracle_and_negative_damping_is_rejected():
+    """NEXT-2 (reading A-20): A_sys = (1/h^2 + c_alpha/h) M + (1 + c_beta/h) L_el + w_vol I."""
+    rest, tris = W.rest_shape("rbc", 2)
+    mat = W.default_material(rest, tris, c_alpha=0.4, c_beta=0.03)
+    plan = NpfemPlan(tris, rest, mat, DT)
+    oc = O.OracleCell(tris, rest, mat, DT)
+    n = rest.shape[0]
+    A = plan.query("system").reshape(n, n)
+    assert np.allclose(A, oc.system_matrix(), rtol=1e-11, atol=1e-12)
+    undamped = NpfemPlan(tris, rest, W.default_material(rest, tris), DT).query("system").reshape(n, n)
+    assert np.abs(A - undamped).max() > 0.1                            # the damping really is in there
+    op = plan.query("operator").reshape(n, n)
+    assert np.abs(op @ A - np.eye(n)).max() < 5e-6
+    with pytest.raises(NpfemError):
+        NpfemPlan(tris, rest, dict(mat, c_beta=-1.0), DT)

@@ -234,3 +234,28 @@ def test_mesh_too_large_for_one_cta_is_rejected_loudly():
     with pytest.raises(NpfemError) as e:
         NpfemHandle(tris, rest, W.default_material(rest, tris), 0.1)
     assert e.value.code == -4
+
+
+@pytest.mark.parametrize("damp", [dict(c_alpha=0.5), dict(c_beta=0.05), dict(c_alpha=0.5, c_beta=0.05)])
+def test_viscoelastic_damping_matches_the_oracle(damp):
+    """NEXT-2 (reading A-20): implicit Rayleigh damping
+    C = c_alpha M + c_beta L_el.  The kernel folds it into the residual (diagonal, membrane and
+    hinge factors) and a once-per-step constant; the oracle adds (C/h) x_n to the right-hand side
+    of the damped system.  Cells start with velocities, so the damping really acts."""
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=7, **damp)
+    vel0 = (vel0 * 50).astype(np.float32)                      # 5e-3 um/us: damping force ~ elastic force
+    g = _G(rest, tris, mat, pos0, vel0)
+    _parity(g, forces * 2, 10)
+    # and it is not a no-op: the damped run differs from the undamped one by far more than the check resolves
+    a = list(gpu_trajectory(g, 0.1, forces, 10))[-1][1]
+    g0 = _G(rest, tris, W.default_material(rest, tris), pos0, vel0)
+    b = list(gpu_trajectory(g0, 0.1, forces, 10))[-1][1]
+    assert np.abs(a - b).max() > 0.02 * np.abs(b).max()
+
+
+def test_damping_on_rbc3_and_platelets_with_world_offsets():
+    for kind, level, n_cells in (("rbc", 3, 6), ("plt", 1, 37)):
+        rest, tris, mat, pos0, vel0, forces = _small_workload(kind=kind, level=level, n_cells=n_cells,
+                                                              c_alpha=0.3, c_beta=0.02)
+        vel0 = (vel0 * 30).astype(np.float32)
+        _parity(_G(rest, tris, mat, pos0, vel0), forces, 12)
