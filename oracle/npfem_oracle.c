@@ -652,6 +652,139 @@ void oracle_step_cell(const oracle_cell *c, double *pos, double *vel, const doub
   free(s); free(x); free(b); free(Ps); free(Pa); free(Pb); free(Pv);
 }
 
+/* ---------------------------------------------------------------- converged solve (NEXT-1)
+ * "Our approach follows the redesigned projective dynamics approach as described
+ * in Liu et al. [11] ... we provide a converged solution"; :133 "unconditional stability for
+ * arbitrary time steps".  Reading A-21: the step minimises the implicit-Euler objective
+ *   g(x) = 1/2 ||x - s||^2_M / h^2 + E_el(x) [+ 1/(2h) (x - x_n)^T C (x - x_n)],
+ *   E_el(x) = sum_t 1/2 w_s dist^2(F_t, strain set) + 1/2 w_a dist^2(F_t, area set)
+ *           + sum_h 1/2 w_h dist^2(k_h, sphere r_h) + 1/2 w_volume dist^2(x, {V = V*}),
+ * whose gradient is  grad g(x) = M (x - s)/h^2 - f_int(x) [+ C (x - x_n)/h]  (the projections
+ * are closest points, so their derivatives drop out), by L-BFGS with the constant, prefactored
+ * A_sys as initial Hessian (two-loop recursion over the last `history` pairs), a backtracking
+ * (halving) line search on g with the Armijo constant 1e-4, and the stop criterion
+ *   res(x) = max_v || (h^2/m_v) grad g(x)_v ||_inf <= tol
+ * (a length: the displacement the unbalanced force would cause in one free step).
+ * history = 0 and line_search = 0 is the plain local/global sweep (pin P-8). */
+
+/* g(x) and its gradient; work arrays are allocated by the caller (Ps,Pa [T][6], Pb [H][3], Pv [n][3]) */
+double oracle_objective(const oracle_cell *c, const double *x, const double *s, const double *xn,
+                        double *grad) {
+  int n = c->n; size_t m3 = 3*(size_t)n; double ih2 = 1.0 / (c->h * c->h);
+  double *Ps = (double*)malloc(sizeof(double)*6*c->T), *Pa = (double*)malloc(sizeof(double)*6*c->T);
+  double *Pb = (double*)malloc(sizeof(double)*3*c->H), *Pv = (double*)malloc(sizeof(double)*m3);
+  oracle_local(c, x, Ps, Pa, Pb, Pv);
+  double gval = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, xn);
+  if (grad) {
+    double *f = (double*)malloc(sizeof(double)*m3), *dmp = (double*)calloc(m3, sizeof(double));
+    oracle_fint(c, x, f);
+    /* C (x - x_n)/h = (C/h) x - (C/h) x_n, with oracle_damping_rhs(v) = (C/h) v */
+    double *tmp = (double*)calloc(m3, sizeof(double));
+    oracle_damping_rhs(c, x, dmp); oracle_damping_rhs(c, xn, tmp);
+    for (int v = 0; v < n; ++v)
+      for (int d = 0; d < 3; ++d)
+        grad[3*v+d] = c->mass[v] * ih2 * (x[3*v+d] - s[3*v+d]) - f[3*v+d] + dmp[3*v+d] - tmp[3*v+d];
+    free(f); free(dmp); free(tmp);
+  }
+  free(Ps); free(Pa); free(Pb); free(Pv);
+  return gval;
+}
+
+static double residual_length(const oracle_cell *c, const double *grad) {
+  double r = 0, h2 = c->h * c->h;
+  for (int v = 0; v < c->n; ++v)
+    for (int d = 0; d < 3; ++d) { double q = fabs(grad[3*v+d]) * h2 / c->mass[v]; if (q > r) r = q; }
+  return r;
+}
+static double dotn(const double *a, const double *b, size_t m) { double s = 0; for (size_t i = 0; i < m; ++i) s += a[i]*b[i]; return s; }
+
+/* One converged time step of ONE cell.  Returns the number of iterations taken.
+ * Optional traces: gtrace[max_iters+1] objective after each accepted iterate (gtrace[0] = g(s)),
+ * rtrace[max_iters+1] residual lengths, iterates [(max_iters+1)][n][3]. */
+int oracle_step_cell_converged(const oracle_cell *c, double *pos, double *vel, const double *fext,
+                               double tol, int max_iters, int history, int line_search,
+                               double *gtrace, double *rtrace, double *iterates) {
+  int n = c->n; size_t m3 = 3*(size_t)n; double h = c->h;
+  if (history < 0) history = 0;
+  double *s = (double*)malloc(sizeof(double)*m3), *x = (double*)malloc(sizeof(double)*m3);
+  double *grad = (double*)malloc(sizeof(double)*m3), *gnew = (double*)malloc(sizeof(double)*m3);
+  double *q = (double*)malloc(sizeof(double)*m3), *r = (double*)malloc(sizeof(double)*m3);
+  double *xt = (double*)malloc(sizeof(double)*m3);
+  double *S = (double*)malloc(sizeof(double)*m3*(size_t)(history ? history : 1));
+  double *Y = (double*)malloc(sizeof(double)*m3*(size_t)(history ? history : 1));
+  double *rho = (double*)malloc(sizeof(double)*(size_t)(history ? history : 1));
+  double *alpha = (double*)malloc(sizeof(double)*(size_t)(history ? history : 1));
+  for (int v = 0; v < n; ++v)
+    for (int d = 0; d < 3; ++d)
+      s[3*v+d] = pos[3*v+d] + h * vel[3*v+d] + h*h * fext[3*v+d] / c->mass[v];
+  memcpy(x, s, sizeof(double)*m3);
+  double gval = oracle_objective(c, x, s, pos, grad);
+  int npairs = 0, k = 0;
+  if (gtrace) gtrace[0] = gval;
+  if (rtrace) rtrace[0] = residual_length(c, grad);
+  if (iterates) memcpy(iterates, x, sizeof(double)*m3);
+  while (k < max_iters && residual_length(c, grad) > tol) {
+    /* two-loop recursion; pair j of age a (0 = newest) sits in slot (k-1-a) % history */
+    memcpy(q, grad, sizeof(double)*m3);
+    for (int a = 0; a < npairs; ++a) {
+      int j = (k - 1 - a) % history;
+      alpha[j] = rho[j] * dotn(S + j*m3, q, m3);
+      for (size_t i = 0; i < m3; ++i) q[i] -= alpha[j] * Y[j*m3 + i];
+    }
+    oracle_solve(c, q, r);                                   /* r = A_sys^-1 q */
+    for (int a = npairs - 1; a >= 0; --a) {
+      int j = (k - 1 - a) % history;
+      double beta = rho[j] * dotn(Y + j*m3, r, m3);
+      for (size_t i = 0; i < m3; ++i) r[i] += S[j*m3 + i] * (alpha[j] - beta);
+    }
+    /* direction p = -r.  The distance energies are only piecewise smooth, so a quasi-Newton
+     * direction can fail to descend: then the history is dropped and p = -A_sys^-1 grad g, which
+     * always descends (A_sys is SPD). */
+    double slope = -dotn(grad, r, m3), step = 1.0, gtry;
+    if (npairs > 0 && !(slope < 0.0)) {
+      npairs = 0;
+      oracle_solve(c, grad, r);
+      slope = -dotn(grad, r, m3);
+    }
+    for (;;) {
+      for (size_t i = 0; i < m3; ++i) xt[i] = x[i] - step * r[i];
+      gtry = oracle_objective(c, xt, s, pos, gnew);
+      /* sufficient decrease, up to the rounding of g itself (near convergence the decrease is
+       * below fp64 resolution of g and an exact test would reject every step) */
+      if (!line_search || gtry <= gval + 1e-4 * step * slope + 8.0 * 2.220446049250313e-16 * fabs(gval) || step < 1e-6) break;
+      step *= 0.5;
+    }
+    if (history > 0) {
+      int j = k % history;
+      double sy = 0;
+      for (size_t i = 0; i < m3; ++i) { S[j*m3+i] = xt[i] - x[i]; Y[j*m3+i] = gnew[i] - grad[i]; sy += S[j*m3+i]*Y[j*m3+i]; }
+      if (sy > 1e-300) { rho[j] = 1.0 / sy; if (npairs < history) ++npairs; }
+      else npairs = 0;                                       /* curvature condition failed: restart */
+    }
+    memcpy(x, xt, sizeof(double)*m3); memcpy(grad, gnew, sizeof(double)*m3); gval = gtry;
+    ++k;
+    if (gtrace) gtrace[k] = gval;
+    if (rtrace) rtrace[k] = residual_length(c, grad);
+    if (iterates) memcpy(iterates + (size_t)k*m3, x, sizeof(double)*m3);
+  }
+  for (size_t i = 0; i < m3; ++i) { vel[i] = (x[i] - pos[i]) / h; pos[i] = x[i]; }
+  free(s); free(x); free(grad); free(gnew); free(q); free(r); free(xt); free(S); free(Y); free(rho); free(alpha);
+  return k;
+}
+
+/* All cells, OpenMP over cells; iters_out[n_cells] receives the iterations each cell took. */
+void oracle_step_converged(const oracle_cell *c, int n_cells, double *pos, double *vel,
+                           const double *fext, double tol, int max_iters, int history,
+                           int32_t *iters_out) {
+  size_t stride = 3*(size_t)c->n;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int i = 0; i < n_cells; ++i) {
+    int it = oracle_step_cell_converged(c, pos + i*stride, vel + i*stride, fext + i*stride, tol,
+                                        max_iters, history, 1, NULL, NULL, NULL);
+    if (iters_out) iters_out[i] = it;
+  }
+}
+
 /* All cells of one type, [n_cells][n][3] fp64 arrays, OpenMP over cells only. */
 void oracle_step(const oracle_cell *c, int n_cells, double *pos, double *vel, const double *fext,
                  int n_iters) {

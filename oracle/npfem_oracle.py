@@ -69,6 +69,13 @@ def lib():
         L.oracle_dissipation.restype = C.c_double
         L.oracle_dissipation.argtypes = [C.c_void_p, _dp, _dp]
         L.oracle_step_cell.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_int, _dp, _dp]
+        L.oracle_objective.restype = C.c_double
+        L.oracle_objective.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
+        L.oracle_step_cell_converged.restype = C.c_int
+        L.oracle_step_cell_converged.argtypes = [C.c_void_p, _dp, _dp, _dp, C.c_double, C.c_int,
+                                                 C.c_int, C.c_int, _dp, _dp, _dp]
+        L.oracle_step_converged.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_double, C.c_int,
+                                            C.c_int, _ip]
         L.oracle_step.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, C.c_int]
         L.oracle_num_threads.restype = C.c_int
         _lib = L
@@ -254,6 +261,42 @@ class OracleCell:
             return pos, vel, its, en
         lib().oracle_step_cell(self._h, _d(pos), _d(vel), _d(fext), int(n_iters), None, None)
         return pos, vel
+
+    # ---- converged solve (NEXT-1, reading A-21)
+    def objective(self, x, s, xn, grad=False):
+        """g(x) of the implicit-Euler step [and its gradient]."""
+        x, s, xn = _f64(x), _f64(s), _f64(xn)
+        if grad:
+            gr = np.empty((self.n, 3))
+            return float(lib().oracle_objective(self._h, _d(x), _d(s), _d(xn), _d(gr))), gr
+        return float(lib().oracle_objective(self._h, _d(x), _d(s), _d(xn), None))
+
+    def step_cell_converged(self, pos, vel, fext, tol, max_iters=200, history=5, line_search=True,
+                            trace=False):
+        """One converged step of one cell: L-BFGS seeded with A_sys^-1 + backtracking line search.
+        Returns (pos, vel, iters[, g_trace, res_trace, iterates])."""
+        pos, vel, fext = _f64(pos).copy(), _f64(vel).copy(), _f64(fext)
+        if trace:
+            gt, rt = np.full(max_iters + 1, np.nan), np.full(max_iters + 1, np.nan)
+            its = np.full((max_iters + 1, self.n, 3), np.nan)
+            k = lib().oracle_step_cell_converged(self._h, _d(pos), _d(vel), _d(fext), float(tol),
+                                                 int(max_iters), int(history), int(line_search),
+                                                 _d(gt), _d(rt), _d(its))
+            return pos, vel, int(k), gt[: k + 1], rt[: k + 1], its[: k + 1]
+        k = lib().oracle_step_cell_converged(self._h, _d(pos), _d(vel), _d(fext), float(tol),
+                                             int(max_iters), int(history), int(line_search),
+                                             None, None, None)
+        return pos, vel, int(k)
+
+    def step_converged(self, pos, vel, fext, tol, max_iters=200, history=5):
+        """One converged step of N cells [N,n,3]; returns (pos, vel, iters[N])."""
+        pos = np.array(pos, dtype=np.float64, order="C", copy=True)
+        vel = np.array(vel, dtype=np.float64, order="C", copy=True)
+        fext = _f64(fext)
+        its = np.zeros(pos.shape[0], dtype=np.int32)
+        lib().oracle_step_converged(self._h, pos.shape[0], _d(pos), _d(vel), _d(fext), float(tol),
+                                    int(max_iters), int(history), _i(its))
+        return pos, vel, its
 
     def step(self, pos, vel, fext, n_iters):
         """One step of N cells, arrays [N,n,3]; fp32 inputs are promoted to fp64. Returns (pos, vel) fp64."""

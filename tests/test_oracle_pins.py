@@ -577,3 +577,93 @@ def test_P16_damping_dissipates_mechanical_energy():
         out[key] = mech_energy(cell, x, v)
     assert out["alpha"] < out["none"] and out["beta"] < out["none"]
     assert out["both"] < min(out["alpha"], out["beta"])
+
+
+# ----------------------------------------------------------------------------- converged solve (A-21)
+def _residual_length(cell, x, s, xn, dt):
+    _, gr = cell.objective(x, s, xn, grad=True)
+    return np.abs(gr * dt ** 2 / cell.masses()[:, None]).max()
+
+
+def test_P17_no_history_unit_step_is_the_plain_local_global_sweep():
+    """PAPER.md:94 via P-8: with no L-BFGS history and no line search the converged-solve driver
+    walks exactly the iterates of the fixed-count step."""
+    c, rest, _, _ = make_cell("rbc", 2)
+    rng = np.random.default_rng(41)
+    x0 = rest + 0.01 * rng.standard_normal(rest.shape)
+    v0 = 1e-3 * rng.standard_normal(rest.shape)
+    f = 5e-3 * rng.standard_normal(rest.shape)
+    K = 6
+    _, _, its_plain, _ = c.step_cell(x0, v0, f, K, trace=True)
+    x, v, k, gt, rt, its = c.step_cell_converged(x0, v0, f, 0.0, K, history=0, line_search=False, trace=True)
+    assert k == K and np.abs(its - its_plain).max() < 1e-13
+    xp, vp = c.step_cell(x0, v0, f, K)
+    assert np.abs(x - xp).max() < 1e-13 and np.abs(v - vp).max() < 1e-11
+
+
+@pytest.mark.parametrize("damp", [{}, dict(c_alpha=0.3, c_beta=0.05)])
+def test_P18_objective_gradient_matches_finite_differences(damp):
+    """grad g = M (x-s)/h^2 - f_int(x) [+ C (x-x_n)/h]: the projections are closest points, so
+    their derivatives drop out (envelope).  Central differences of g on random coordinates."""
+    c, rest, _, _ = make_cell("plt", 1, s_min=0.9, s_max=1.1, a_min=0.95, a_max=1.05, **damp)
+    rng = np.random.default_rng(42)
+    xn = rest + 0.02 * rng.standard_normal(rest.shape)
+    s = xn + 0.01 * rng.standard_normal(rest.shape)
+    x = xn + 0.03 * rng.standard_normal(rest.shape)
+    g0, gr = c.objective(x, s, xn, grad=True)
+    assert g0 > 0
+    eps = 1e-6
+    for _ in range(12):
+        i, d = rng.integers(rest.shape[0]), rng.integers(3)
+        e = np.zeros_like(x); e[i, d] = eps
+        fd = (c.objective(x + e, s, xn) - c.objective(x - e, s, xn)) / (2 * eps)
+        assert fd == pytest.approx(gr[i, d], rel=2e-5, abs=1e-9)
+
+
+@pytest.mark.parametrize("dt", [0.1, 1.0, 10.0])
+def test_P19_objective_decreases_at_every_accepted_step(dt):
+    rest, tris = W.rest_shape("rbc", 2)
+    c = O.OracleCell(tris, rest, W.default_material(rest, tris), dt)
+    rng = np.random.default_rng(43)
+    f = 1e-3 * rng.standard_normal(rest.shape)
+    x, v, k, gt, rt, _ = c.step_cell_converged(rest * 1.03, np.zeros_like(rest), f, 1e-9, 400, 3, True, trace=True)
+    assert k >= 3
+    assert (np.diff(gt) <= 1e-12 * np.abs(gt[:-1])).all()
+    assert rt[-1] < 1e-3 * rt[0]
+
+
+def test_P20_converged_state_is_the_limit_of_plain_sweeps():
+    c, rest, _, _ = make_cell("rbc", 2)
+    rng = np.random.default_rng(44)
+    x0 = rest + 0.01 * rng.standard_normal(rest.shape)
+    f = 5e-3 * rng.standard_normal(rest.shape)
+    z = np.zeros_like(rest)
+    x_lim, _ = c.step_cell(x0, z, f, 250)
+    x, v, k = c.step_cell_converged(x0, z, f, 1e-12, 200, history=5)
+    assert k < 60
+    assert np.abs(x - x_lim).max() < 1e-10
+    s = x0 + DT ** 2 * f / c.masses()[:, None]
+    assert _residual_length(c, x, s, x0, DT) <= 1e-12
+
+
+@pytest.mark.parametrize("scale", [10, 100])
+def test_P21_large_time_steps_converge_where_20_fixed_sweeps_do_not(scale):
+    """PAPER.md:133 "unconditional stability for arbitrary time steps": at dt x 10 and x 100 the
+    inertial diagonal no longer dominates, 20 plain sweeps leave a large unbalanced force, the
+    quasi-Newton iteration with line search still reaches the tolerance."""
+    dt = DT * scale
+    rest, tris = W.rest_shape("rbc", 2)
+    c = O.OracleCell(tris, rest, W.default_material(rest, tris), dt)
+    rng = np.random.default_rng(45)
+    f = 1e-3 * rng.standard_normal(rest.shape)
+    z = np.zeros_like(rest)
+    x0 = rest * 1.02
+    s = x0 + dt ** 2 * f / c.masses()[:, None]
+    tol = 1e-7
+    x20, _ = c.step_cell(x0, z, f, 20)
+    x, v, k = c.step_cell_converged(x0, z, f, tol, 3000, history=5)
+    r20, rc = _residual_length(c, x20, s, x0, dt), _residual_length(c, x, s, x0, dt)
+    assert rc <= tol and r20 > 100 * tol
+    # and the history pays: far fewer iterations than the same driver without it
+    _, _, k0 = c.step_cell_converged(x0, z, f, tol, 3000, history=0)
+    assert k < 0.5 * k0
