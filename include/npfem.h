@@ -120,6 +120,26 @@ int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float*
                int n_iters, void* cuda_stream);
 
 /*
+ * npfem_step_converged: advance n_cells cells by ONE time step solved to convergence (PAPER.md:94-95
+ * "redesigned projective dynamics approach as described in Liu et al. ... we provide a converged
+ * solution"; :133 "unconditional stability for arbitrary time steps"; reading A-21): per
+ * cell, L-BFGS (3 pairs) seeded with the prefactored A_sys^-1 and a backtracking line search on the
+ * implicit-Euler objective g(x) = 1/2 ||x - s||^2_M/h^2 + E_el(x), until
+ *     res = max_v || (h^2/m_v) grad g(x)_v ||_inf <= tol      (a length, caller's unit)
+ * or max_iters iterations.  One kernel launch, one CTA per cell, the stop flag lives on the device.
+ *   pos, vel, fext  device, as for npfem_step
+ *   tol             >= 0; fp32 resolves about 1e-7 x the cell radius
+ *   max_iters       >= 0
+ *   iters_out       device, int32 [n_cells] or NULL: iterations each cell took
+ *   res_out         device, float [n_cells] or NULL: final residual length of each cell
+ *   cuda_stream     as for npfem_step
+ * Errors: NPFEM_EINVAL (also: handle created with damping, not supported here yet), NPFEM_ECUDA.
+ */
+int npfem_step_converged(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+                         double tol, int max_iters, int32_t* iters_out, float* res_out,
+                         void* cuda_stream);
+
+/*
  * npfem_step_host: the same step with HOST buffers (pinned or pageable): cells are cut into
  * chunks that flow host->device, through the step kernel and device->host on three streams so
  * copies overlap compute.  Blocking: returns when pos/vel hold the new state (also on error: no

@@ -65,6 +65,8 @@ def load_library(path: str | None = None):
                                  C.c_int, C.c_int, C.POINTER(Options), C.POINTER(vp)]
     lib.npfem_step.restype = C.c_int
     lib.npfem_step.argtypes = [vp, C.c_int, fp, fp, fp, C.c_int, vp]
+    lib.npfem_step_converged.restype = C.c_int
+    lib.npfem_step_converged.argtypes = [vp, C.c_int, fp, fp, fp, C.c_double, C.c_int, vp, vp, vp]
     lib.npfem_step_host.restype = C.c_int
     lib.npfem_step_host.argtypes = [vp, C.c_int, fp, fp, fp, C.c_int]
     lib.npfem_destroy.restype = C.c_int
@@ -146,6 +148,11 @@ def npfem_step(handle: "NpfemHandle", n_cells: int, pos, vel, fext, n_iters: int
     return handle.step(n_cells, pos, vel, fext, n_iters, stream)
 
 
+def npfem_step_converged(handle: "NpfemHandle", n_cells: int, pos, vel, fext, tol: float,
+                         max_iters: int, iters_out=None, res_out=None, stream=None):
+    handle.step_converged(n_cells, pos, vel, fext, tol, max_iters, iters_out, res_out, stream)
+
+
 def npfem_step_host(handle: "NpfemHandle", n_cells: int, pos, vel, fext, n_iters: int):
     return handle.step_host(n_cells, pos, vel, fext, n_iters)
 
@@ -185,6 +192,16 @@ class NpfemHandle:
         s = 0 if stream is None else int(getattr(stream, "cuda_stream", stream))
         _check(load_library().npfem_step(self._h, int(n_cells), _ptr(pos), _ptr(vel), _ptr(fext),
                                          int(n_iters), s))
+
+    def step_converged(self, n_cells: int, pos, vel, fext, tol: float, max_iters: int,
+                       iters_out=None, res_out=None, stream=None):
+        """Converged quasi-Newton step (npfem_step_converged); iters_out int32 / res_out float32
+        device arrays [n_cells] or None.  Asynchronous on `stream`."""
+        s = 0 if stream is None else int(getattr(stream, "cuda_stream", stream))
+        _check(load_library().npfem_step_converged(
+            self._h, int(n_cells), _ptr(pos), _ptr(vel), _ptr(fext), float(tol), int(max_iters),
+            _ptr(iters_out) if iters_out is not None else None,
+            _ptr(res_out) if res_out is not None else None, s))
 
     def step_host(self, n_cells: int, pos, vel, fext, n_iters: int):
         _check(load_library().npfem_step_host(self._h, int(n_cells), _ptr(pos), _ptr(vel),

@@ -13,8 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnpfem_b200.so")
-SOURCES = ["npfem_plan.cpp", "npfem_kernels.cu", "npfem_api.cu", "npfem_peak.cu"]
-HEADERS = ["npfem_internal.h", "npfem_kernels.cuh", os.path.join(ROOT, "include", "npfem.h")]
+SOURCES = ["npfem_plan.cpp", "npfem_kernels.cu", "npfem_api.cu", "npfem_peak.cu", "npfem_converged.cu"]
+HEADERS = ["npfem_internal.h", "npfem_kernels.cuh", "npfem_device.cuh", os.path.join(ROOT, "include", "npfem.h")]
 
 
 def _nvcc() -> str:

@@ -233,6 +233,7 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   cudaError_t e = cudaGetDevice(&H->device);
   if (e != cudaSuccess) { delete H; return cuda_err(e, "cudaGetDevice (no CUDA device: there is no CPU fallback)"); }
   e = configure_kernels(P.smem_bytes);
+  if (e == cudaSuccess) e = configure_converged_kernels();
   if (e != cudaSuccess) { delete H; return cuda_err(e, "cudaFuncSetAttribute(shared memory)"); }
 
   // ---- one blob for all constant tables, 256-byte aligned sections
@@ -353,6 +354,28 @@ int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float*
   cudaError_t e = launch_step(p, h->plan.threads, h->plan.smem_bytes, h->plan.global_mode,
                               static_cast<cudaStream_t>(cuda_stream));
   if (e != cudaSuccess) return cuda_err(e, "npfem_step launch");
+  return NPFEM_OK;
+}
+
+int npfem_step_converged(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+                         double tol, int max_iters, int32_t* iters_out, float* res_out,
+                         void* cuda_stream) {
+  if (!h) return set_err(NPFEM_EINVAL, "null handle");
+  if (n_cells < 0 || max_iters < 0 || !(tol >= 0.0)) return set_err(NPFEM_EINVAL, "negative n_cells, max_iters or tol");
+  if (n_cells == 0) return NPFEM_OK;
+  if (!pos || !vel || !fext) return set_err(NPFEM_EINVAL, "null device pointer");
+  if (h->max_cells > 0 && n_cells > h->max_cells) return set_err(NPFEM_EINVAL, "n_cells exceeds the max_cells given to npfem_create");
+  if (h->plan.damped) return set_err(NPFEM_EINVAL, "the converged solve does not support damping yet (c_alpha, c_beta must be 0)");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_err(guard.err, "cudaSetDevice(handle device)");
+  DevParams p = h->dev;
+  p.n_cells = n_cells; p.n_iters = max_iters;
+  p.pos = pos; p.vel = vel; p.fext = fext;
+  p.k = 1;                                               // one CTA owns one cell
+  p.L = smem_layout(h->plan.n, h->plan.E, h->plan.nvb, 1);
+  cudaError_t e = launch_converged(p, h->plan.threads, p.L.total, (float)tol, max_iters, iters_out, res_out,
+                                   static_cast<cudaStream_t>(cuda_stream));
+  if (e != cudaSuccess) return cuda_err(e, "npfem_step_converged launch");
   return NPFEM_OK;
 }
 

@@ -47,4 +47,10 @@ cudaError_t configure_kernels(int smem_bytes);
 cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mode,
                         cudaStream_t stream);
 
+// Converged quasi-Newton step (npfem_converged.cu): one CTA per cell; p.k must be 1 and p.L the
+// shared-memory layout for k = 1.  iters_out / res_out: device arrays [n_cells] or NULL.
+cudaError_t configure_converged_kernels();
+cudaError_t launch_converged(const DevParams& p, int threads, int smem_bytes, float tol, int max_iters,
+                             int* iters_out, float* res_out, cudaStream_t stream);
+
 }  // namespace npfem

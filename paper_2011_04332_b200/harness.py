@@ -48,6 +48,14 @@ class DeviceGroup:
     def step(self, n_iters: int, stream=None):
         self.handle.step(self.n_cells, self.pos, self.vel, self.fext, n_iters, stream)
 
+    def step_converged(self, tol: float, max_iters: int, stream=None):
+        """Converged quasi-Newton step; returns (iterations, residual lengths) per cell (numpy)."""
+        its = torch.zeros(self.n_cells, dtype=torch.int32, device=self.device)
+        res = torch.zeros(self.n_cells, dtype=torch.float32, device=self.device)
+        self.handle.step_converged(self.n_cells, self.pos, self.vel, self.fext, tol, max_iters, its, res, stream)
+        torch.cuda.synchronize()
+        return its.cpu().numpy(), res.cpu().numpy()
+
     def state(self):
         torch.cuda.synchronize()
         return (from_strided(self.pos, self.n_verts), from_strided(self.vel, self.n_verts))
