@@ -75,6 +75,10 @@ typedef struct {
   int global_mode;        /* 0 = auto, 1 = fp32 SIMT blocks, 2 = 3xTF32 tensor-core blocks          */
   int pair_triangles;     /* local-step work items: 0 = auto / 1 = pairs of triangles across a shared */
                           /* edge wherever the matching finds one, 2 = one triangle per item        */
+  int debug_jitter;       /* 0 = off; otherwise a seed: every warp of the step kernel sleeps a      */
+                          /* pseudo-random time (< 2 us) after every CTA barrier.  Results must be  */
+                          /* bit-identical to debug_jitter = 0; a difference means a missing barrier */
+                          /* (schedule-fuzz race check; costs time, never use it in production)     */
 } npfem_options;
 
 /*

@@ -30,7 +30,8 @@ class Material(C.Structure):
 
 class Options(C.Structure):
     _fields_ = [("inv_drop_tol", C.c_double), ("volume_inner_iters", C.c_int),
-                ("cells_per_cta", C.c_int), ("global_mode", C.c_int), ("pair_triangles", C.c_int)]
+                ("cells_per_cta", C.c_int), ("global_mode", C.c_int), ("pair_triangles", C.c_int),
+                ("debug_jitter", C.c_int)]
 
 
 class Info(C.Structure):
@@ -115,9 +116,9 @@ def _material(mat: dict) -> Material:
 
 
 def _options(inv_drop_tol=None, volume_inner_iters=0, cells_per_cta=0, global_mode=0,
-             pair_triangles=0) -> Options:
+             pair_triangles=0, debug_jitter=0) -> Options:
     return Options(-1.0 if inv_drop_tol is None else float(inv_drop_tol), int(volume_inner_iters),
-                   int(cells_per_cta), int(global_mode), int(pair_triangles))
+                   int(cells_per_cta), int(global_mode), int(pair_triangles), int(debug_jitter))
 
 
 def _mesh_args(tris, rest_xyz):

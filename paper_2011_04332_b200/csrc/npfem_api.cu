@@ -319,6 +319,7 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.damp_m = reinterpret_cast<const float*>(base + secs[12].off);
   D.cbh = (float)(P.mat.c_beta / P.h);
   D.damped = P.damped ? 1 : 0;
+  D.jitter = P.opt.debug_jitter;
   D.L = smem_layout(n, E, P.nvb, P.cells_per_cta);
   if (max_cells > 0) {   // everything any later step entry point needs exists now
     rc = create_pipeline(H, max_cells);

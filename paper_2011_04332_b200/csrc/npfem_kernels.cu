@@ -29,6 +29,22 @@
 namespace npfem {
 namespace {
 
+// Debug option `debug_jitter` (npfem_options): every warp sleeps a pseudo-random time after every
+// CTA barrier, so that warps cross each phase at very different times.  A missing barrier between
+// a phase that writes a shared buffer and one that reads it then changes the result, while a
+// correctly synchronised kernel stays bit-identical (tests/test_edge_cases_gpu.py) -- the stand-in
+// for compute-sanitizer racecheck, which is closed on this pool.
+__device__ __forceinline__ void jitter_sleep(int seed, int phase, int warp) {
+  unsigned hsh = ((unsigned)seed * 2654435761u) ^ ((unsigned)phase * 40503u) ^ ((unsigned)warp * 9176u + blockIdx.x * 7u);
+  hsh ^= hsh >> 13; hsh *= 0x5bd1e995u; hsh ^= hsh >> 15;
+  __nanosleep(hsh & 2047u);
+}
+#define NPFEM_SYNC()                                                    \
+  do {                                                                  \
+    __syncthreads();                                                    \
+    if (P.jitter) jitter_sleep(P.jitter, ++jphase, warp);               \
+  } while (0)
+
 // ------------------------------------------------------------------------------------------
 // The fused step kernel.  MODE 1: global step with fp32 FMAs (comparison path); MODE 2: 3xTF32
 // mma.sync on the block-sparse inverse.
@@ -46,6 +62,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+  int jphase = 0;   // barrier counter of the schedule-jitter debug option
   const int n = P.n, E = P.E, nvb = P.nvb, NP = nvb * 8;
   const int cell0 = blockIdx.x * P.k;
   const int kact = min(P.k, P.n_cells - cell0);
@@ -78,7 +95,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     reinterpret_cast<float4*>(z4b)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  __syncthreads();
+  NPFEM_SYNC();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t ta = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * kTmemGroup);
 
@@ -99,7 +116,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         for (int i = tid; i < n3; i += blockDim.x) {
           st[i] = P.pos[g + i]; st[n3 + i] = P.vel[g + i]; st[2 * n3 + i] = P.fext[g + i];
         }
-        __syncthreads();
+        NPFEM_SYNC();
         float sx = 0.f, sy = 0.f, sz = 0.f;
         if (isv) {
 #pragma unroll
@@ -111,7 +128,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         }
         sx = warp_sum(sx); sy = warp_sum(sy); sz = warp_sum(sz);
         if (lane == 0) red[c * 32 + warp] = make_float4(sx, sy, sz, 0.f);
-        __syncthreads();   // staging is reused by the next cell; partial sums complete
+        NPFEM_SYNC();   // staging is reused by the next cell; partial sums complete
       }
     }
 #pragma unroll
@@ -133,7 +150,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     tmem_st16(ta + 16, zero16);
     tmem_st16(ta + 32, zero16);
     tmem_st16(ta + 48, ur);
-    __syncthreads();
+    NPFEM_SYNC();
     if (DAMP) {
       // Rayleigh damping, implicit (reading A-20): the damping force -(C/h)(x - x_n),
       // C = c_alpha M + c_beta L_el, with x - x_n = u0 + d and L_el (u0 + d) = L_el z - L_el y:
@@ -155,10 +172,10 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
             float4* z4c = reinterpret_cast<float4*>(z4b) + c * NP;
             if (isv) z4c[v] = make_float4(sreg[3 * c] - ur[3 * c], sreg[3 * c + 1] - ur[3 * c + 1],
                                           sreg[3 * c + 2] - ur[3 * c + 2], 0.f);        // y = s - u0
-            __syncthreads();
+            NPFEM_SYNC();
             if (tid < E)
               element_residual<2>(ecs + tid, E, z4b + c * cellz, P, reinterpret_cast<float4*>(rbb) + tid);
-            __syncthreads();
+            NPFEM_SYNC();
             if (isv) {
               F3 q = {0.f, 0.f, 0.f};
               const uint32_t ioff[kRegList / 2] = {vr0q.x, vr0q.y, vr0q.z};
@@ -172,7 +189,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
               qreg[3 * c] = q.x; qreg[3 * c + 1] = q.y; qreg[3 * c + 2] = q.z;
               z4c[v] = make_float4(sreg[3 * c], sreg[3 * c + 1], sreg[3 * c + 2], 0.f);   // back to z = s
             }
-            __syncthreads();
+            NPFEM_SYNC();
           }
         }
       }
@@ -220,7 +237,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       }
     };
     elements_and_gradient(0);
-    __syncthreads();
+    NPFEM_SYNC();
     for (int c = 0; c < kact; ++c) {
       const unsigned char* zc = z4b + c * cellz;
       const unsigned char* outb = (c & 1) ? rab : rbb;
@@ -267,7 +284,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           const F3 zz = zv + D;
           if (isv) z4c[v] = make_float4(zz.x, zz.y, zz.z, 0.f);
           moved = true;
-          __syncthreads();
+          NPFEM_SYNC();
           float S3 = 0.f;
           S1 = 0.f; S2 = 0.f;
           if (isv) {
@@ -277,7 +294,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           }
           S1 = warp_sum(S1); S2 = warp_sum(S2); S3 = warp_sum(S3);
           if (lane == 0) red[c * 32 + warp] = make_float4(S1, S2, S3, 0.f);
-          __syncthreads();
+          NPFEM_SYNC();
           p4 = lane < nwarps ? red[c * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
           S1 = warp_sum(p4.x); S2 = warp_sum(p4.y); S3 = warp_sum(p4.z);
           C = S1 * (1.0f / 3.0f) - vstar;
@@ -286,7 +303,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           const float D2new = lambda * lambda * S2;
           more = (D2new + D2prev - 2.0f * lambda * S3) > vol_dtol2;
           D2prev = D2new;
-          __syncthreads();   // red[c] is rewritten by the next pass
+          NPFEM_SYNC();   // red[c] is rewritten by the next pass
         }
         if (moved && isv) reinterpret_cast<float4*>(z4b + c * cellz)[v] = make_float4(zv.x, zv.y, zv.z, 0.f);
       }
@@ -296,7 +313,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       tmem_st4(ta + 32 + 3 * c, fmaf(P.w_volume, D.x, ev.x), fmaf(P.w_volume, D.y, ev.y),
                fmaf(P.w_volume, D.z, ev.z), 0.0f);
       if (c + 1 < kact) elements_and_gradient(c + 1);
-      __syncthreads();   // out(c) consumed; out(c+1) and the partial sums of cell c+1 complete
+      NPFEM_SYNC();   // out(c) consumed; out(c+1) and the partial sums of cell c+1 complete
     }
 
     // right-hand sides of the global step, r = e - (m/h^2) d, split into tf32 high and low parts and
@@ -323,7 +340,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         }
       }
     }
-    __syncthreads();
+    NPFEM_SYNC();
 
     // global step: delta d = T r with T = A_sys^-1 in 8x8 blocks.  One warp per block row of 8
     // output vertices (up to 4 rows per warp): mma m16n8k8, M = the 16 right-hand-side columns,
@@ -366,7 +383,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         }
       }
     }
-    __syncthreads();   // every warp is done reading the right-hand sides
+    NPFEM_SYNC();   // every warp is done reading the right-hand sides
 
     // hand the increments to the vertex owners: dd[m][NP] over the dead lo buffer
 #pragma unroll
@@ -378,7 +395,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         if (g8 < 7) *reinterpret_cast<float2*>(rb + (g8 + 8) * NP + i0) = make_float2(acc[j][2], acc[j][3]);
       }
     }
-    __syncthreads();
+    NPFEM_SYNC();
 
     // owner update: d += delta d, z = s + d
     {
@@ -396,7 +413,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       }
       tmem_st16(ta + 16, dv);
     }
-    __syncthreads();
+    NPFEM_SYNC();
   }
 
   // ---- epilogue: x_n+1 = x_n + (u0 + d), v_n+1 = (u0 + d)/h, staged in caller order through
@@ -413,7 +430,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       if (c < kact) {
         const size_t g = (size_t)(cell0 + c) * P.cell_stride;
         for (int i = tid; i < n3; i += blockDim.x) st[i] = P.pos[g + i];
-        __syncthreads();
+        NPFEM_SYNC();
         if (isv) {
 #pragma unroll
           for (int q = 0; q < 3; ++q) {
@@ -422,14 +439,14 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
             st[n3 + vext3 + q] = inc * invh;
           }
         }
-        __syncthreads();
+        NPFEM_SYNC();
         for (int i = tid; i < n3; i += blockDim.x) { P.pos[g + i] = st[i]; P.vel[g + i] = st[n3 + i]; }
-        __syncthreads();
+        NPFEM_SYNC();
       }
     }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  __syncthreads();
+  NPFEM_SYNC();
   if (warp == 0)
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base_s), "r"(tmem_cols) : "memory");
 }

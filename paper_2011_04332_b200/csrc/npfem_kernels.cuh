@@ -21,6 +21,7 @@ struct DevParams {
   float s_min, s_max, a_min, a_max;
   float cbh;                               // c_beta / h (stiffness-proportional damping, A-20)
   int damped;                              // c_alpha != 0 or c_beta != 0
+  int jitter;                              // debug: seed of the per-warp sleeps after every barrier (0 = off)
   const uint16_t* perm;                    // [NP] internal -> caller vertex (padding: 0)
   const float4* elem_c;                    // [kElemGroups][E] element constants (npfem_api.cu)
   const float* h2_over_m;                  // [NP]

@@ -136,6 +136,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     o.cells_per_cta = opts->cells_per_cta;
     o.global_mode = opts->global_mode;
     o.pair_triangles = opts->pair_triangles;
+    o.debug_jitter = opts->debug_jitter;
   }
   if (o.volume_inner_iters <= 0) o.volume_inner_iters = 8;
   if (o.volume_inner_iters > 32) o.volume_inner_iters = 32;

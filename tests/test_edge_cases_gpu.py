@@ -259,3 +259,33 @@ def test_damping_on_rbc3_and_platelets_with_world_offsets():
                                                               c_alpha=0.3, c_beta=0.02)
         vel0 = (vel0 * 30).astype(np.float32)
         _parity(_G(rest, tris, mat, pos0, vel0), forces, 12)
+
+
+def test_schedule_jitter_leaves_results_bit_identical():
+    """Race check by schedule fuzzing (compute-sanitizer is closed on this pool): with
+    debug_jitter every warp sleeps a pseudo-random time after every CTA barrier, so warps cross
+    the kernel's phases (two shared buffers with three lives each per iteration, the temporary
+    overwrite of z in the volume passes, the staging buffers) at very different times.  Any
+    missing barrier would let a fast warp overwrite what a slow warp still reads; a correctly
+    synchronised kernel is bit-identical for every seed."""
+    cases = []
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=7)
+    cases += [("rbc2 k=5", rest, tris, mat, pos0, vel0, forces, {}),
+              ("rbc2 k=2", rest, tris, mat, pos0, vel0, forces, dict(cells_per_cta=2)),
+              ("rbc2 single triangles", rest, tris, mat, pos0, vel0, forces, dict(pair_triangles=2)),
+              ("rbc2 simt", rest, tris, mat, pos0, vel0, forces, dict(global_mode=1))]
+    c = pos0.mean(axis=1, keepdims=True)
+    shrunk = (c + (pos0 - c) * 0.9).astype(np.float32)
+    cases.append(("rbc2 shrunk (volume passes)", rest, tris, mat, shrunk, np.zeros_like(pos0), forces, {}))
+    matd = W.default_material(rest, tris, c_alpha=0.3, c_beta=0.03)
+    cases.append(("rbc2 damped", rest, tris, matd, pos0, vel0, forces, {}))
+    r3 = _small_workload(level=3, n_cells=6)
+    cases.append(("rbc3", r3[0], r3[1], r3[2], r3[3], r3[4], r3[5], {}))
+    pl = _small_workload(kind="plt", level=1, n_cells=23)
+    cases.append(("plt", pl[0], pl[1], pl[2], pl[3], pl[4], pl[5], {}))
+    for name, rest, tris, mat, pos0, vel0, forces, opt in cases:
+        g = _G(rest, tris, mat, pos0, vel0)
+        ref = list(gpu_trajectory(g, 0.1, forces[:2], 6, **opt))[-1]
+        for seed in (1, 2, 3):
+            out = list(gpu_trajectory(g, 0.1, forces[:2], 6, debug_jitter=seed, **opt))[-1]
+            assert np.array_equal(ref[0], out[0]) and np.array_equal(ref[1], out[1]), (name, seed)
