@@ -59,6 +59,9 @@ typedef struct {
                                  /* >= 0: implicit Rayleigh damping f_d = -(c_alpha M + c_beta L_el) */
                                  /* v_{n+1}, L_el = the strain + area + bending stiffness (A-20);    */
                                  /* c_alpha in 1/time, c_beta in time                                */
+  double w_collision;            /* collision weight per vertex (PAPER.md:145 collisions_weight), >= 0; */
+  double d_collision;            /* contact distance >= 0: a vertex with a colliding neighbour (q, n)   */
+                                 /* is kept at (x - q).n >= d_collision (reading A-22); both 0 = off   */
 } npfem_material;
 
 /* Tuning knobs that do not change what is computed beyond fp32 rounding.  Pass NULL for defaults. */

@@ -50,6 +50,7 @@ typedef struct {
   double k_bend;
   double w_volume, v_min, v_max;
   double c_alpha, c_beta;
+  double w_collision, d_collision;   /* collision weight per vertex, contact distance (reading A-22) */
 } oracle_material;
 
 typedef struct oracle_cell {
@@ -320,6 +321,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   if (n < 4 || T < 4 || !tris || !X || !mat || !(h > 0)) return ORACLE_EINVAL;
   if (mat->s_min > mat->s_max || mat->a_min > mat->a_max || mat->v_min > mat->v_max) return ORACLE_EINVAL;
   if (mat->c_alpha < 0.0 || mat->c_beta < 0.0) return ORACLE_EINVAL;
+  if (mat->w_collision < 0.0 || mat->d_collision < 0.0) return ORACLE_EINVAL;
   if (!(mat->cell_mass > 0)) return ORACLE_EINVAL;
   for (int i = 0; i < 3*T; ++i) if (tris[i] < 0 || tris[i] >= n) return ORACLE_EINVAL;
   if ((3*T) % 2) return ORACLE_EINVAL;
@@ -420,7 +422,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   if (!(c->V0 > 0)) { oracle_destroy(c); return ORACLE_EINVAL; }
 
   /* step 5: L_el = sum_t (w_s+w_a) G^T G + sum_h w_h K^T K;
-   *         A_sys = (1/h^2 + c_alpha/h) diag(m) + (1 + c_beta/h) L_el + w_volume I
+   *         A_sys = (1/h^2 + c_alpha/h) diag(m) + (1 + c_beta/h) L_el + (w_volume + w_collision) I
    * (c_alpha = c_beta = 0: the undamped system of SURVEY.md 8(c); otherwise reading A-20: the
    * Rayleigh damping force -(c_alpha M + c_beta L_el)(x - x_n)/h of implicit Euler moves
    * (c_alpha M + c_beta L_el)/h to the left-hand side) */
@@ -439,7 +441,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   }
   for (size_t i = 0; i < (size_t)n*n; ++i) c->A[i] = (1.0 + mat->c_beta / h) * c->Lel[i];
   for (int v = 0; v < n; ++v)
-    c->A[(size_t)v*n+v] += c->mass[v] * (1.0/(h*h) + mat->c_alpha / h) + mat->w_volume;
+    c->A[(size_t)v*n+v] += c->mass[v] * (1.0/(h*h) + mat->c_alpha / h) + mat->w_volume + mat->w_collision;
   if (chol_dense(n, c->A, c->L) != 0) { oracle_destroy(c); return ORACLE_EINVAL; }
   for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) c->LT[(size_t)j*n+i] = c->L[(size_t)i*n+j];
   *out = c;
@@ -589,6 +591,91 @@ void oracle_fint(const oracle_cell *c, const double *x, double *f) {
     }
   (void)m;
   free(Ps); free(Pa); free(Pb); free(Pv); free(zero);
+}
+
+void oracle_damping_rhs(const oracle_cell *c, const double *xn, double *b);
+double oracle_dissipation(const oracle_cell *c, const double *x, const double *xn);
+
+/* ---------------------------------------------------------------- collisions (NEXT-3, reading A-22)
+ * the coupling hands "external forces & colliding neighbours" to the solid solver;
+ * :145 "collision forces intensity (collisions_weight parameter)".  Reading: per vertex at most one
+ * colliding neighbour per step, given as a point q on the other body and that body's outward unit
+ * normal nrm at q (nrm = 0: no neighbour).  The vertex must stay on the outer side of the plane,
+ * at least d_collision away:  (x_v - q).nrm >= d.  Projection (closest point of that half space):
+ *   t = d - (x_v - q).nrm;   p = x_v + max(t, 0) nrm.
+ * Energy 1/2 w_collision ||x_v - p||^2 with selection matrix I, so w_collision sits on the diagonal
+ * of A_sys for EVERY vertex (inactive vertices project onto themselves and feel no force), which
+ * keeps the system matrix constant while contacts come and go. */
+void oracle_project_collision(const double *x, const double *q, const double *nrm, double d, double *p) {
+  double t = d - ((x[0]-q[0])*nrm[0] + (x[1]-q[1])*nrm[1] + (x[2]-q[2])*nrm[2]);
+  if (!(t > 0.0) || (nrm[0] == 0.0 && nrm[1] == 0.0 && nrm[2] == 0.0)) t = 0.0;
+  p[0] = x[0] + t*nrm[0]; p[1] = x[1] + t*nrm[1]; p[2] = x[2] + t*nrm[2];
+}
+/* all vertices: Pc [n][3]; returns the collision energy 1/2 w_c sum ||x - Pc||^2 */
+double oracle_collision_local(const oracle_cell *c, const double *x, const double *q, const double *nrm,
+                              double *Pc) {
+  double e = 0;
+  for (int v = 0; v < c->n; ++v) {
+    oracle_project_collision(x + 3*v, q + 3*v, nrm + 3*v, c->mat.d_collision, Pc + 3*v);
+    for (int d = 0; d < 3; ++d) e += (x[3*v+d]-Pc[3*v+d])*(x[3*v+d]-Pc[3*v+d]);
+  }
+  return 0.5 * c->mat.w_collision * e;
+}
+
+/* One time step of ONE cell with colliding neighbours (q, nrm: [n][3], held fixed over the step):
+ * the local/global sweeps of oracle_step_cell with the collision projections added to the rhs.
+ * energies [2*n_iters] as in oracle_step_cell (collision energy included). */
+void oracle_step_cell_collide(const oracle_cell *c, double *pos, double *vel, const double *fext,
+                              const double *q, const double *nrm, int n_iters, double *iterates,
+                              double *energies) {
+  int n = c->n; size_t m3 = 3*(size_t)n; double h = c->h, wc = c->mat.w_collision;
+  double *s = (double*)malloc(sizeof(double)*m3), *x = (double*)malloc(sizeof(double)*m3);
+  double *b = (double*)malloc(sizeof(double)*m3), *Pc = (double*)malloc(sizeof(double)*m3);
+  double *Ps = (double*)malloc(sizeof(double)*6*c->T), *Pa = (double*)malloc(sizeof(double)*6*c->T);
+  double *Pb = (double*)malloc(sizeof(double)*3*c->H), *Pv = (double*)malloc(sizeof(double)*m3);
+  for (int v = 0; v < n; ++v)
+    for (int d = 0; d < 3; ++d)
+      s[3*v+d] = pos[3*v+d] + h * vel[3*v+d] + h*h * fext[3*v+d] / c->mass[v];
+  memcpy(x, s, sizeof(double)*m3);
+  if (iterates) memcpy(iterates, x, sizeof(double)*m3);
+  for (int k = 0; k < n_iters; ++k) {
+    oracle_local(c, x, Ps, Pa, Pb, Pv);
+    double ec = oracle_collision_local(c, x, q, nrm, Pc);
+    if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + ec;
+    oracle_rhs(c, s, Ps, Pa, Pb, Pv, b);
+    oracle_damping_rhs(c, pos, b);
+    for (size_t i = 0; i < m3; ++i) b[i] += wc * Pc[i];
+    oracle_solve(c, b, x);
+    if (energies) {
+      double e2 = 0;
+      for (size_t i = 0; i < m3; ++i) e2 += (x[i]-Pc[i])*(x[i]-Pc[i]);
+      energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + 0.5*wc*e2;
+    }
+    if (iterates) memcpy(iterates + (size_t)(k+1)*m3, x, sizeof(double)*m3);
+  }
+  for (size_t i = 0; i < m3; ++i) { vel[i] = (x[i] - pos[i]) / h; pos[i] = x[i]; }
+  free(s); free(x); free(b); free(Pc); free(Ps); free(Pa); free(Pb); free(Pv);
+}
+void oracle_step_collide(const oracle_cell *c, int n_cells, double *pos, double *vel, const double *fext,
+                         const double *q, const double *nrm, int n_iters) {
+  size_t stride = 3*(size_t)c->n;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int i = 0; i < n_cells; ++i)
+    oracle_step_cell_collide(c, pos + i*stride, vel + i*stride, fext + i*stride, q + i*stride,
+                             nrm + i*stride, n_iters, NULL, NULL);
+}
+
+/* area per surface vertex at the current configuration (consumed by the IBM):
+ * a_v = 1/3 sum over the triangles around v of their area */
+void oracle_vertex_areas(const oracle_cell *c, const double *x, double *a) {
+  for (int v = 0; v < c->n; ++v) a[v] = 0.0;
+  for (int t = 0; t < c->T; ++t) {
+    const int32_t *tr = c->tris + 3*t;
+    double e1[3], e2[3], cr[3];
+    sub3(x + 3*tr[1], x + 3*tr[0], e1); sub3(x + 3*tr[2], x + 3*tr[0], e2); cross3(e1, e2, cr);
+    double A = 0.5 * norm3(cr);
+    for (int e = 0; e < 3; ++e) a[tr[e]] += A / 3.0;
+  }
 }
 
 /* Rayleigh damping, implicit (reading A-20): C = c_alpha M + c_beta L_el, f_d = -C (x - x_n)/h.

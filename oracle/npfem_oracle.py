@@ -15,7 +15,8 @@ import numpy as np
 from . import build as _build
 
 MATERIAL_FIELDS = ("cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min", "a_max",
-                   "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta")
+                   "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta", "w_collision",
+                   "d_collision")
 
 
 class _Material(C.Structure):
@@ -65,6 +66,10 @@ def lib():
         L.oracle_energy.restype = C.c_double
         L.oracle_energy.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
         L.oracle_fint.argtypes = [C.c_void_p, _dp, _dp]
+        L.oracle_project_collision.argtypes = [_dp, _dp, _dp, C.c_double, _dp]
+        L.oracle_step_cell_collide.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp, C.c_int, _dp, _dp]
+        L.oracle_step_collide.argtypes = [C.c_void_p, C.c_int, _dp, _dp, _dp, _dp, _dp, C.c_int]
+        L.oracle_vertex_areas.argtypes = [C.c_void_p, _dp, _dp]
         L.oracle_damping_rhs.argtypes = [C.c_void_p, _dp, _dp]
         L.oracle_dissipation.restype = C.c_double
         L.oracle_dissipation.argtypes = [C.c_void_p, _dp, _dp]
@@ -133,6 +138,12 @@ def project_bend(k, r):
     return P
 
 
+def project_collision(x, q, nrm, d):
+    x, q, nrm = _f64(x, (3,)), _f64(q, (3,)), _f64(nrm, (3,)); p = np.empty(3)
+    lib().oracle_project_collision(_d(x), _d(q), _d(nrm), float(d), _d(p))
+    return p
+
+
 def volume(tris, x):
     tris = np.ascontiguousarray(tris, dtype=np.int32); x = _f64(x)
     return float(lib().oracle_volume(tris.shape[0], _i(tris), _d(x)))
@@ -164,7 +175,7 @@ class OracleCell:
         self.T = self.tris.shape[0]
         self.dt = float(dt)
         self.material = dict(material)
-        m = _Material(**{k: float(material[k]) for k in MATERIAL_FIELDS})
+        m = _Material(**{k: float(material.get(k, 0.0)) for k in MATERIAL_FIELDS})
         h = C.c_void_p()
         rc = lib().oracle_create(self.n, self.T, _i(self.tris), _d(self.rest), C.byref(m),
                                  self.dt, C.byref(h))
@@ -261,6 +272,31 @@ class OracleCell:
             return pos, vel, its, en
         lib().oracle_step_cell(self._h, _d(pos), _d(vel), _d(fext), int(n_iters), None, None)
         return pos, vel
+
+    # ---- collisions and area per vertex (NEXT-3, reading A-22)
+    def step_cell_collide(self, pos, vel, fext, q, nrm, n_iters, trace=False):
+        pos, vel, fext = _f64(pos).copy(), _f64(vel).copy(), _f64(fext)
+        q, nrm = _f64(q), _f64(nrm)
+        if trace:
+            its = np.empty((n_iters + 1, self.n, 3)); en = np.empty(2 * n_iters)
+            lib().oracle_step_cell_collide(self._h, _d(pos), _d(vel), _d(fext), _d(q), _d(nrm),
+                                           int(n_iters), _d(its), _d(en))
+            return pos, vel, its, en
+        lib().oracle_step_cell_collide(self._h, _d(pos), _d(vel), _d(fext), _d(q), _d(nrm),
+                                       int(n_iters), None, None)
+        return pos, vel
+
+    def step_collide(self, pos, vel, fext, q, nrm, n_iters):
+        pos = np.array(pos, dtype=np.float64, order="C", copy=True)
+        vel = np.array(vel, dtype=np.float64, order="C", copy=True)
+        fext, q, nrm = _f64(fext), _f64(q), _f64(nrm)
+        lib().oracle_step_collide(self._h, pos.shape[0], _d(pos), _d(vel), _d(fext), _d(q), _d(nrm),
+                                  int(n_iters))
+        return pos, vel
+
+    def vertex_areas(self, x):
+        x = _f64(x); a = np.empty(self.n)
+        lib().oracle_vertex_areas(self._h, _d(x), _d(a)); return a
 
     # ---- converged solve (NEXT-1, reading A-21)
     def objective(self, x, s, xn, grad=False):

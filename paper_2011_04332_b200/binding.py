@@ -13,7 +13,8 @@ import numpy as np
 from . import build as _build
 
 MATERIAL_FIELDS = ("cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min", "a_max",
-                   "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta")
+                   "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta", "w_collision",
+                   "d_collision")
 
 QUERY = {"perm": (1, np.int32), "mass": (2, np.float64), "system": (3, np.float64),
          "operator": (4, np.float64), "hinge_verts": (5, np.int32), "hinge_K": (6, np.float64),
@@ -112,7 +113,7 @@ def _check(rc: int):
 
 
 def _material(mat: dict) -> Material:
-    return Material(**{k: float(mat[k]) for k in MATERIAL_FIELDS})
+    return Material(**{k: float(mat.get(k, 0.0)) for k in MATERIAL_FIELDS})
 
 
 def _options(inv_drop_tol=None, volume_inner_iters=0, cells_per_cta=0, global_mode=0,

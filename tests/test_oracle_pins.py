@@ -667,3 +667,90 @@ def test_P21_large_time_steps_converge_where_20_fixed_sweeps_do_not(scale):
     # and the history pays: far fewer iterations than the same driver without it
     _, _, k0 = c.step_cell_converged(x0, z, f, tol, 3000, history=0)
     assert k < 0.5 * k0
+
+
+# ----------------------------------------------------------------------------- collisions, areas (A-22)
+def test_P22_collision_projection_is_the_closest_point_of_the_half_space():
+    rng = np.random.default_rng(51)
+    for _ in range(40):
+        x, q = rng.standard_normal(3), rng.standard_normal(3)
+        nrm = rng.standard_normal(3); nrm /= np.linalg.norm(nrm)
+        d = rng.uniform(0.0, 0.5)
+        p = O.project_collision(x, q, nrm, d)
+        assert (p - q) @ nrm >= d - 1e-12                               # feasible
+        if (x - q) @ nrm >= d:
+            assert np.array_equal(p, x)                                 # inactive: no force
+        # brute force: no feasible sample is closer
+        cand = x + rng.standard_normal((4000, 3)) * (np.linalg.norm(p - x) + 0.1)
+        feas = cand[(cand - q) @ nrm >= d]
+        if len(feas):
+            assert np.linalg.norm(p - x) <= np.linalg.norm(feas - x, axis=1).min() + 1e-12
+    assert np.array_equal(O.project_collision(np.ones(3), np.zeros(3), np.zeros(3), 0.3), np.ones(3))
+
+
+def test_P23_free_cell_pressed_against_a_wall_settles_at_the_closed_form_penetration():
+    """No elasticity, constant force f on every vertex towards a wall (every vertex has the wall as
+    colliding neighbour): static equilibrium w_c (d - gap) = |f|  =>  gap = d - |f|/w_c."""
+    rest, tris = W.rest_shape("plt", 1)
+    wc, d, fmag = 2.0, 0.05, 1e-2
+    mat = W.default_material(rest, tris, k_strain=0, k_area=0, k_bend=0, w_volume=0, c_alpha=2.0,
+                             w_collision=wc, d_collision=d)
+    c = O.OracleCell(tris, rest, mat, DT)
+    n = rest.shape[0]
+    nrm = np.tile([0.0, 0.0, 1.0], (n, 1))                               # wall z = 0, outward normal +z
+    q = np.zeros((n, 3))
+    f = np.tile([0.0, 0.0, -fmag], (n, 1))
+    x = rest + np.array([0.0, 0.0, 0.5 - rest[:, 2].min()])              # lowest vertex 0.5 above the wall
+    v = np.zeros_like(x)
+    for _ in range(4000):
+        x, v = c.step_cell_collide(x, v, f, q, nrm, 3)
+    assert np.abs(v).max() < 1e-9
+    assert np.abs(x[:, 2] - (d - fmag / wc)).max() < 1e-8                # every vertex: same gap (no elasticity)
+
+
+def test_P24_collide_step_identities():
+    """(i) no active neighbour: identical to the plain step although w_c sits on the diagonal;
+    (ii) one sweep = x - A_sys^-1 grad of the objective with the collision energy
+    (iii) the objective is monotone over the local/global half steps (P-3 with collisions)."""
+    c, rest, _, mat = make_cell("rbc", 2, w_collision=1.5, d_collision=0.02)
+    c0, _, _, _ = make_cell("rbc", 2)
+    rng = np.random.default_rng(52)
+    x0 = rest + 0.01 * rng.standard_normal(rest.shape)
+    v0 = 1e-3 * rng.standard_normal(rest.shape)
+    f = 5e-3 * rng.standard_normal(rest.shape)
+    n = rest.shape[0]
+    zero = np.zeros_like(rest)
+    xa, va = c.step_cell_collide(x0, v0, f, zero, zero, 5)
+    xb, vb = c0.step_cell(x0, v0, f, 5)
+    assert np.abs(xa - xb).max() < 1e-6        # same fixed point, different (both contracting) iterations
+    xa, _ = c.step_cell_collide(x0, v0, f, zero, zero, 60)
+    xb, _ = c0.step_cell(x0, v0, f, 60)
+    assert np.abs(xa - xb).max() < 1e-12
+    # a plane cutting through the cell: about half of the vertices active
+    nrm = np.tile([1.0, 0.0, 0.0], (n, 1)); q = np.tile([0.5, 0.0, 0.0], (n, 1))
+    _, _, its, en = c.step_cell_collide(x0, v0, f, q, nrm, 6, trace=True)
+    assert (np.diff(en) <= 1e-12 * np.abs(en[:-1])).all()
+    m = c.masses()[:, None]
+    s = its[0]
+    A = c.system_matrix()
+    assert np.allclose(np.diag(A) - np.diag(c0.system_matrix()), 1.5)
+    for k in range(6):
+        Pc = np.array([O.project_collision(its[k][i], q[i], nrm[i], 0.02) for i in range(n)])
+        active = ((its[k] - q) * nrm).sum(axis=1) < 0.02
+        assert 0.2 * n < active.sum() < 0.8 * n or k > 0
+        grad = m * (its[k] - s) / DT ** 2 - c.fint(its[k]) + 1.5 * (its[k] - Pc)
+        pred = its[k] - c.solve(grad)
+        assert np.abs(pred - its[k + 1]).max() < 1e-12
+
+
+def test_P25_vertex_areas():
+    """a_v = 1/3 of the areas of the triangles around v: sums to the surface area (unit icosphere
+    -> 4 pi from below), equals the lumped-mass share at rest, scales with the square of a scaling."""
+    c, rest, tris, mat = make_cell("rbc", 3)
+    a = c.vertex_areas(rest)
+    assert a.sum() == pytest.approx(c.areas().sum(), rel=1e-13)
+    assert np.allclose(a / a.sum(), c.masses() / c.masses().sum(), rtol=1e-12)
+    assert np.allclose(c.vertex_areas(1.7 * rest), 1.7 ** 2 * a, rtol=1e-12)
+    sph, st = W.mesh.icosphere(3)
+    cs = O.OracleCell(st, sph, W.default_material(sph, st), DT)
+    assert 0.98 * 4 * np.pi < cs.vertex_areas(sph).sum() < 4 * np.pi

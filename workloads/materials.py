@@ -26,6 +26,7 @@ def default_material(rest_xyz, tris, **overrides) -> dict:
         k_bend=2e-4,
         w_volume=0.5, v_min=1.0, v_max=1.0,
         c_alpha=0.0, c_beta=0.0,
+        w_collision=0.0, d_collision=0.0,
     )
     for k, v in overrides.items():
         if k not in mat:
