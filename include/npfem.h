@@ -127,6 +127,31 @@ int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float*
                int n_iters, void* cuda_stream);
 
 /*
+ * npfem_step_collide: npfem_step with colliding neighbours (the coupling hands
+ * "external forces & colliding neighbours" to the solid solver; :129-133 cell packing; :145
+ * collisions_weight; reading A-22).  Per vertex at most one neighbour: a point q on the
+ * other body and that body's outward unit normal n at q; the vertex is kept on the outer side,
+ * (x - q).n >= d_collision, by a projective constraint of weight w_collision (both in the
+ * material given to npfem_create; w_collision sits on the diagonal of A_sys for every vertex, so
+ * contacts may come and go without touching the prefactored system).  Neighbour detection is the
+ * caller's (the paper's framework does it outside npFEM); q and n are held fixed over the step.
+ *   coll_q, coll_n  device, float, in, [n_cells][cell_stride], vertex-major xyz like pos;
+ *                   n = (0,0,0) marks a vertex without neighbour
+ * Everything else as npfem_step.
+ */
+int npfem_step_collide(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+                       const float* coll_q, const float* coll_n, int n_iters, void* cuda_stream);
+
+/*
+ * npfem_vertex_areas: area per surface vertex at the given positions, a_v = 1/3 of the areas of the
+ * triangles around v -- what the immersed-boundary coupling needs from the solid side
+ * (PAPER.md:226).  One small kernel, asynchronous on the stream.
+ *   pos     device, float, in, [n_cells][cell_stride]
+ *   areas   device, float, out, [n_cells][n_verts] (caller's vertex order)
+ */
+int npfem_vertex_areas(npfem_handle h, int n_cells, const float* pos, float* areas, void* cuda_stream);
+
+/*
  * npfem_step_converged: advance n_cells cells by ONE time step solved to convergence (PAPER.md:94-95
  * "redesigned projective dynamics approach as described in Liu et al. ... we provide a converged
  * solution"; :133 "unconditional stability for arbitrary time steps"; reading A-21): per
@@ -140,7 +165,8 @@ int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float*
  *   iters_out       device, int32 [n_cells] or NULL: iterations each cell took
  *   res_out         device, float [n_cells] or NULL: final residual length of each cell
  *   cuda_stream     as for npfem_step
- * Errors: NPFEM_EINVAL (also: handle created with damping, not supported here yet), NPFEM_ECUDA.
+ * Errors: NPFEM_EINVAL (also: handle created with damping or collisions, not supported here yet),
+ * NPFEM_ECUDA.
  */
 int npfem_step_converged(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
                          double tol, int max_iters, int32_t* iters_out, float* res_out,

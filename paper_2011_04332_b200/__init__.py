@@ -5,9 +5,11 @@ package only marshals arguments.  There is no CPU fallback: creating a handle wi
 device raises.
 """
 from .binding import (NpfemError, NpfemHandle, NpfemPlan, load_library, npfem_create,
-                      npfem_destroy, npfem_step, npfem_step_converged, npfem_step_host, npfem_last_error,
+                      npfem_destroy, npfem_step, npfem_step_collide, npfem_step_converged, npfem_step_host,
+                      npfem_vertex_areas, npfem_last_error,
                       npfem_cell_stride, npfem_measure_fp32_peak, MATERIAL_FIELDS, QUERY)
 
 __all__ = ["NpfemError", "NpfemHandle", "NpfemPlan", "load_library", "npfem_create",
-           "npfem_destroy", "npfem_step", "npfem_step_converged", "npfem_step_host", "npfem_last_error",
+           "npfem_destroy", "npfem_step", "npfem_step_collide", "npfem_step_converged", "npfem_step_host",
+           "npfem_vertex_areas", "npfem_last_error",
            "npfem_cell_stride", "npfem_measure_fp32_peak", "MATERIAL_FIELDS", "QUERY"]

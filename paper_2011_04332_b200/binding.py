@@ -67,6 +67,10 @@ def load_library(path: str | None = None):
                                  C.c_int, C.c_int, C.POINTER(Options), C.POINTER(vp)]
     lib.npfem_step.restype = C.c_int
     lib.npfem_step.argtypes = [vp, C.c_int, fp, fp, fp, C.c_int, vp]
+    lib.npfem_step_collide.restype = C.c_int
+    lib.npfem_step_collide.argtypes = [vp, C.c_int, fp, fp, fp, fp, fp, C.c_int, vp]
+    lib.npfem_vertex_areas.restype = C.c_int
+    lib.npfem_vertex_areas.argtypes = [vp, C.c_int, fp, fp, vp]
     lib.npfem_step_converged.restype = C.c_int
     lib.npfem_step_converged.argtypes = [vp, C.c_int, fp, fp, fp, C.c_double, C.c_int, vp, vp, vp]
     lib.npfem_step_host.restype = C.c_int
@@ -150,6 +154,15 @@ def npfem_step(handle: "NpfemHandle", n_cells: int, pos, vel, fext, n_iters: int
     return handle.step(n_cells, pos, vel, fext, n_iters, stream)
 
 
+def npfem_step_collide(handle: "NpfemHandle", n_cells: int, pos, vel, fext, coll_q, coll_n,
+                       n_iters: int, stream=None):
+    handle.step_collide(n_cells, pos, vel, fext, coll_q, coll_n, n_iters, stream)
+
+
+def npfem_vertex_areas(handle: "NpfemHandle", n_cells: int, pos, areas, stream=None):
+    handle.vertex_areas(n_cells, pos, areas, stream)
+
+
 def npfem_step_converged(handle: "NpfemHandle", n_cells: int, pos, vel, fext, tol: float,
                          max_iters: int, iters_out=None, res_out=None, stream=None):
     handle.step_converged(n_cells, pos, vel, fext, tol, max_iters, iters_out, res_out, stream)
@@ -194,6 +207,16 @@ class NpfemHandle:
         s = 0 if stream is None else int(getattr(stream, "cuda_stream", stream))
         _check(load_library().npfem_step(self._h, int(n_cells), _ptr(pos), _ptr(vel), _ptr(fext),
                                          int(n_iters), s))
+
+    def step_collide(self, n_cells: int, pos, vel, fext, coll_q, coll_n, n_iters: int, stream=None):
+        """npfem_step with one colliding neighbour (point, outward normal; zero normal = none) per vertex."""
+        s = 0 if stream is None else int(getattr(stream, "cuda_stream", stream))
+        _check(load_library().npfem_step_collide(self._h, int(n_cells), _ptr(pos), _ptr(vel), _ptr(fext),
+                                                 _ptr(coll_q), _ptr(coll_n), int(n_iters), s))
+
+    def vertex_areas(self, n_cells: int, pos, areas, stream=None):
+        s = 0 if stream is None else int(getattr(stream, "cuda_stream", stream))
+        _check(load_library().npfem_vertex_areas(self._h, int(n_cells), _ptr(pos), _ptr(areas), s))
 
     def step_converged(self, n_cells: int, pos, vel, fext, tol: float, max_iters: int,
                        iters_out=None, res_out=None, stream=None):

@@ -320,6 +320,8 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.cbh = (float)(P.mat.c_beta / P.h);
   D.damped = P.damped ? 1 : 0;
   D.jitter = P.opt.debug_jitter;
+  D.coll_q = nullptr; D.coll_n = nullptr;
+  D.w_coll = (float)P.mat.w_collision; D.d_coll = (float)P.mat.d_collision;
   D.L = smem_layout(n, E, P.nvb, P.cells_per_cta);
   if (max_cells > 0) {   // everything any later step entry point needs exists now
     rc = create_pipeline(H, max_cells);
@@ -358,6 +360,40 @@ int npfem_step(npfem_handle h, int n_cells, float* pos, float* vel, const float*
   return NPFEM_OK;
 }
 
+int npfem_step_collide(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
+                       const float* coll_q, const float* coll_n, int n_iters, void* cuda_stream) {
+  if (!h) return set_err(NPFEM_EINVAL, "null handle");
+  if (n_cells < 0 || n_iters < 0) return set_err(NPFEM_EINVAL, "negative n_cells or n_iters");
+  if (n_cells == 0) return NPFEM_OK;
+  if (!pos || !vel || !fext || !coll_q || !coll_n) return set_err(NPFEM_EINVAL, "null device pointer");
+  if (h->max_cells > 0 && n_cells > h->max_cells) return set_err(NPFEM_EINVAL, "n_cells exceeds the max_cells given to npfem_create");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_err(guard.err, "cudaSetDevice(handle device)");
+  DevParams p = h->dev;
+  p.n_cells = n_cells; p.n_iters = n_iters;
+  p.pos = pos; p.vel = vel; p.fext = fext;
+  p.coll_q = coll_q; p.coll_n = coll_n;
+  cudaError_t e = launch_step(p, h->plan.threads, h->plan.smem_bytes, h->plan.global_mode,
+                              static_cast<cudaStream_t>(cuda_stream));
+  if (e != cudaSuccess) return cuda_err(e, "npfem_step_collide launch");
+  return NPFEM_OK;
+}
+
+int npfem_vertex_areas(npfem_handle h, int n_cells, const float* pos, float* areas, void* cuda_stream) {
+  if (!h) return set_err(NPFEM_EINVAL, "null handle");
+  if (n_cells < 0) return set_err(NPFEM_EINVAL, "negative n_cells");
+  if (n_cells == 0) return NPFEM_OK;
+  if (!pos || !areas) return set_err(NPFEM_EINVAL, "null device pointer");
+  DeviceGuard guard(h->device);
+  if (guard.err != cudaSuccess) return cuda_err(guard.err, "cudaSetDevice(handle device)");
+  DevParams p = h->dev;
+  p.n_cells = n_cells;
+  p.pos = const_cast<float*>(pos);
+  cudaError_t e = launch_vertex_areas(p, h->plan.threads, areas, static_cast<cudaStream_t>(cuda_stream));
+  if (e != cudaSuccess) return cuda_err(e, "npfem_vertex_areas launch");
+  return NPFEM_OK;
+}
+
 int npfem_step_converged(npfem_handle h, int n_cells, float* pos, float* vel, const float* fext,
                          double tol, int max_iters, int32_t* iters_out, float* res_out,
                          void* cuda_stream) {
@@ -367,6 +403,7 @@ int npfem_step_converged(npfem_handle h, int n_cells, float* pos, float* vel, co
   if (!pos || !vel || !fext) return set_err(NPFEM_EINVAL, "null device pointer");
   if (h->max_cells > 0 && n_cells > h->max_cells) return set_err(NPFEM_EINVAL, "n_cells exceeds the max_cells given to npfem_create");
   if (h->plan.damped) return set_err(NPFEM_EINVAL, "the converged solve does not support damping yet (c_alpha, c_beta must be 0)");
+  if (h->plan.mat.w_collision != 0.0) return set_err(NPFEM_EINVAL, "the converged solve does not support collisions yet (w_collision must be 0)");
   DeviceGuard guard(h->device);
   if (guard.err != cudaSuccess) return cuda_err(guard.err, "cudaSetDevice(handle device)");
   DevParams p = h->dev;

@@ -94,7 +94,7 @@ int build_plan(int n_verts, int n_tris, const int32_t* tris, const double* rest_
 //                         A-fragment order ([nvb][32] float4)
 //   rb   max(E*64, NP*64) element results of the EVEN cells during the local step, then the
 //                         tf32 low parts of the right-hand sides, then the increments of d
-//   red  [5][32] float4   per-warp partial sums of the volume reductions
+//   red  [5][32] float4   per-warp partial sums of the volume reductions, then [5] float4 centroids
 // The inertial prediction s and the correction d are private to the thread that owns the vertex
 // and live in tensor memory (TMEM), 32 columns per group of 4 warps.
 constexpr int kElemGroups = 9;
@@ -111,7 +111,7 @@ inline SmemLayout smem_layout(int n, int E, int nvb, int k) {
   const int rbuf = E * 64 > NP * 64 ? E * 64 : NP * 64;   // both buffers hold [4][E] element results
   L.ra = off; off += rbuf;
   L.rb = off; off += rbuf;
-  L.red = off; off += kMaxCellsPerCta * 32 * 16;
+  L.red = off; off += kMaxCellsPerCta * 32 * 16 + kMaxCellsPerCta * 16;   // + the cells' centroids
   L.total = off;
   return L;
 }

@@ -42,15 +42,18 @@ __device__ __forceinline__ void jitter_sleep(int seed, int phase, int warp) {
 #define NPFEM_SYNC()                                                    \
   do {                                                                  \
     __syncthreads();                                                    \
-    if (P.jitter) jitter_sleep(P.jitter, ++jphase, warp);               \
+    if (OPT && P.jitter) jitter_sleep(P.jitter, ++jphase, warp);        \
   } while (0)
 
 // ------------------------------------------------------------------------------------------
 // The fused step kernel.  MODE 1: global step with fp32 FMAs (comparison path); MODE 2: 3xTF32
 // mma.sync on the block-sparse inverse.
 // ------------------------------------------------------------------------------------------
-template <int MODE, int MAXT, bool DAMP>
+// FEAT 0: the lean kernel of the headline path; FEAT 1: damping (compile-time) plus the run-time
+// options; FEAT 2: undamped with the run-time options (collision neighbours, debug_jitter).
+template <int MODE, int MAXT, int FEAT>
 __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) {
+  constexpr bool DAMP = FEAT == 1, OPT = FEAT != 0;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   unsigned char* const z4b = smem_raw + P.L.z4;                        // [k][NP] float4 iterate z
   const float4* const ecs = reinterpret_cast<const float4*>(smem_raw + P.L.ec);   // element constants
@@ -137,6 +140,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         const float4 p4 = lane < nwarps ? red[c * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
         const float invn = 1.0f / (float)n;
         const float cx = warp_sum(p4.x) * invn, cy = warp_sum(p4.y) * invn, cz = warp_sum(p4.z) * invn;
+        if (OPT && tid == 0) red[kMaxCellsPerCta * 32 + c] = make_float4(cx, cy, cz, 0.f);   // kept for the collision planes
         if (isv) {
           const float sx = (xr[3 * c] - cx) + ur[3 * c];
           const float sy = (xr[3 * c + 1] - cy) + ur[3 * c + 1];
@@ -307,6 +311,19 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         }
         if (moved && isv) reinterpret_cast<float4*>(z4b + c * cellz)[v] = make_float4(zv.x, zv.y, zv.z, 0.f);
       }
+      // colliding neighbour of this vertex (reading A-22): the half space (x - q).n >= d, residual
+      // w_c max(d - (z - q).n, 0) n; q arrives in world coordinates, the iterate is cell-local
+      if (OPT && P.coll_n != nullptr && isv) {
+        const size_t gq = (size_t)(cell0 + c) * P.cell_stride + vext3;
+        const F3 nn = {P.coll_n[gq], P.coll_n[gq + 1], P.coll_n[gq + 2]};
+        if (nn.x != 0.f || nn.y != 0.f || nn.z != 0.f) {
+          const float4 cen = red[kMaxCellsPerCta * 32 + c];
+          const F3 ql = {P.coll_q[gq] - cen.x, P.coll_q[gq + 1] - cen.y, P.coll_q[gq + 2] - cen.z};
+          const F3 zc3 = lds3(zc, v * 16);
+          const float t = P.d_coll - dot(zc3 - ql, nn);
+          if (t > 0.f) ev = fma3(P.w_coll * t, nn, ev);
+        }
+      }
       // elastic residual of the cell's vertices, e = sum of element results + w_vol D, parked in
       // the owner's TMEM columns 32 + 3c .. (the fourth column written belongs to the next cell,
       // which overwrites it later in this same pass)
@@ -451,18 +468,47 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base_s), "r"(tmem_cols) : "memory");
 }
 
+// Area per surface vertex (the IBM needs it): a_v = 1/3 of the areas of the triangles
+// around v = 1/6 sum over the fan of |(r_i - x_v) x (r_i+1 - x_v)|.  One CTA per cell, thread =
+// vertex (internal numbering: ring lists), positions straight from global memory.
+__global__ void npfem_area_kernel(const DevParams P, float* __restrict__ areas) {
+  const int v = threadIdx.x, cell = blockIdx.x;
+  if (v >= P.n) return;
+  const float* x = P.pos + (size_t)cell * P.cell_stride;
+  auto at = [&](int internal) { const int e = 3 * (int)P.perm[internal]; return F3{x[e], x[e + 1], x[e + 2]}; };
+  const F3 xv = at(v);
+  const int r0 = P.ring_ptr[v], r1 = P.ring_ptr[v + 1];
+  const F3 e0 = at(P.ring_off[r0] >> 4) - xv;
+  F3 ep = e0;
+  float a = 0.f;
+  for (int i = r0 + 1; i <= r1; ++i) {
+    const F3 e = i < r1 ? at(P.ring_off[i] >> 4) - xv : e0;
+    const F3 cr = cross_acc(ep, e, F3{0.f, 0.f, 0.f});
+    a += sqrtf(dot(cr, cr));
+    ep = e;
+  }
+  areas[(size_t)cell * P.n + P.perm[v]] = a * (1.0f / 6.0f);
+}
+
 }  // namespace
+
+cudaError_t launch_vertex_areas(const DevParams& p, int threads, float* areas, cudaStream_t stream) {
+  if (p.n_cells <= 0) return cudaSuccess;
+  npfem_area_kernel<<<p.n_cells, threads, 0, stream>>>(p, areas);
+  return cudaGetLastError();
+}
 
 cudaError_t configure_kernels(int smem_bytes) {
   cudaError_t e;
   (void)smem_bytes;
   smem_bytes = kSmemMaxDynamic;   // opt in once to the largest carve-out any cell type may need
-#define NPFEM_CFG(MODE, MAXT, DAMP)                                                             \
-  e = cudaFuncSetAttribute(npfem_step_kernel<MODE, MAXT, DAMP>,                                 \
+#define NPFEM_CFG(MODE, MAXT, FEAT)                                                             \
+  e = cudaFuncSetAttribute(npfem_step_kernel<MODE, MAXT, FEAT>,                                 \
                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);            \
   if (e != cudaSuccess) return e;
-  NPFEM_CFG(1, 672, false) NPFEM_CFG(1, 1024, false) NPFEM_CFG(2, 672, false) NPFEM_CFG(2, 1024, false)
-  NPFEM_CFG(1, 672, true) NPFEM_CFG(1, 1024, true) NPFEM_CFG(2, 672, true) NPFEM_CFG(2, 1024, true)
+  NPFEM_CFG(1, 672, 0) NPFEM_CFG(1, 1024, 0) NPFEM_CFG(2, 672, 0) NPFEM_CFG(2, 1024, 0)
+  NPFEM_CFG(1, 672, 1) NPFEM_CFG(1, 1024, 1) NPFEM_CFG(2, 672, 1) NPFEM_CFG(2, 1024, 1)
+  NPFEM_CFG(1, 672, 2) NPFEM_CFG(1, 1024, 2) NPFEM_CFG(2, 672, 2) NPFEM_CFG(2, 1024, 2)
 #undef NPFEM_CFG
   return cudaSuccess;
 }
@@ -471,10 +517,12 @@ cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mod
                         cudaStream_t stream) {
   if (p.n_cells <= 0) return cudaSuccess;
   const int grid = (p.n_cells + p.k - 1) / p.k;
-#define NPFEM_LAUNCH(MODE, MAXT)                                                                \
-  do {                                                                                          \
-    if (p.damped) npfem_step_kernel<MODE, MAXT, true><<<grid, threads, smem_bytes, stream>>>(p); \
-    else npfem_step_kernel<MODE, MAXT, false><<<grid, threads, smem_bytes, stream>>>(p);        \
+  const int feat = p.damped ? 1 : (p.coll_n != nullptr || p.jitter != 0) ? 2 : 0;
+#define NPFEM_LAUNCH(MODE, MAXT)                                                                  \
+  do {                                                                                            \
+    if (feat == 1) npfem_step_kernel<MODE, MAXT, 1><<<grid, threads, smem_bytes, stream>>>(p);    \
+    else if (feat == 2) npfem_step_kernel<MODE, MAXT, 2><<<grid, threads, smem_bytes, stream>>>(p); \
+    else npfem_step_kernel<MODE, MAXT, 0><<<grid, threads, smem_bytes, stream>>>(p);              \
   } while (0)
   if (threads <= 672) {
     if (mode == 2) NPFEM_LAUNCH(2, 672); else NPFEM_LAUNCH(1, 672);

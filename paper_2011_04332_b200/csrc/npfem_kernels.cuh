@@ -38,6 +38,9 @@ struct DevParams {
   float* pos;
   float* vel;
   const float* fext;
+  const float* coll_q;                     // [n_cells][cell_stride] colliding neighbour point per vertex, or NULL
+  const float* coll_n;                     // [n_cells][cell_stride] its outward unit normal (0 = none), or NULL
+  float w_coll, d_coll;                    // collision weight, contact distance (A-22)
   SmemLayout L;
 };
 
@@ -47,6 +50,9 @@ cudaError_t configure_kernels(int smem_bytes);
 // Enqueue one step on `stream`.  threads = CTA size (multiple of 32), mode 1 = SIMT, 2 = 3xTF32.
 cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mode,
                         cudaStream_t stream);
+
+// Area per surface vertex at the current positions: areas [n_cells][n] in caller order.
+cudaError_t launch_vertex_areas(const DevParams& p, int threads, float* areas, cudaStream_t stream);
 
 // Converged quasi-Newton step (npfem_converged.cu): one CTA per cell; p.k must be 1 and p.L the
 // shared-memory layout for k = 1.  iters_out / res_out: device arrays [n_cells] or NULL.

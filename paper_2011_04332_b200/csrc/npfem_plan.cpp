@@ -120,6 +120,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     return fail(NPFEM_EINVAL, "clamp band with min > max");
   if (!(mat->c_alpha >= 0.0) || !(mat->c_beta >= 0.0))
     return fail(NPFEM_EINVAL, "damping coefficients c_alpha, c_beta must be >= 0 (DESIGN.md A-20)");
+  if (!(mat->w_collision >= 0.0) || !(mat->d_collision >= 0.0))
+    return fail(NPFEM_EINVAL, "collision weight and contact distance must be >= 0 (DESIGN.md A-22)");
   if (!(mat->cell_mass > 0.0)) return fail(NPFEM_EINVAL, "cell_mass must be positive");
   if (mat->k_strain < 0 || mat->k_area < 0 || mat->k_bend < 0 || mat->w_volume < 0)
     return fail(NPFEM_EINVAL, "negative weight");
@@ -237,7 +239,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     }
   if (hc != H) return fail(NPFEM_EINVAL, "edge count does not match 3T/2");
 
-  // ---- A_sys (caller order) = (1/h^2 + c_alpha/h) M + (1 + c_beta/h) L_el + w_volume I, where
+  // ---- A_sys (caller order) = (1/h^2 + c_alpha/h) M + (1 + c_beta/h) L_el + (w_volume + w_collision) I, where
   //      L_el = sum_t (w_s + w_a) G^T G + sum_h w_h K^T K.  c_alpha = c_beta = 0: the undamped
   //      system; otherwise the implicit Rayleigh damping of reading A-20
   const double ih2 = 1.0 / (dt * dt);
@@ -261,7 +263,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
       for (int q = 0; q < 4; ++q) A[(size_t)hv[p] * n + hv[q]] += wh * K[p] * K[q];
   }
   for (double& a : A) a *= el_scale;
-  for (int v = 0; v < n; ++v) A[(size_t)v * n + v] += P->mass[v] * mass_scale + mat->w_volume;
+  for (int v = 0; v < n; ++v) A[(size_t)v * n + v] += P->mass[v] * mass_scale + mat->w_volume + mat->w_collision;
 
   // ---- T = A_sys^-1 (fp64): Cholesky A = L L^T, M = L^-1, T = M^T M
   std::vector<double> L((size_t)n * n, 0.0), M((size_t)n * n, 0.0), Tinv((size_t)n * n, 0.0);

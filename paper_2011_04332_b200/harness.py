@@ -48,6 +48,19 @@ class DeviceGroup:
     def step(self, n_iters: int, stream=None):
         self.handle.step(self.n_cells, self.pos, self.vel, self.fext, n_iters, stream)
 
+    def step_collide(self, coll_q, coll_n, n_iters: int, stream=None):
+        """coll_q, coll_n: [N,V,3] arrays (numpy or torch); zero normal = no neighbour."""
+        q = to_strided(coll_q, self.stride, self.device)
+        nn = to_strided(coll_n, self.stride, self.device)
+        self.handle.step_collide(self.n_cells, self.pos, self.vel, self.fext, q, nn, n_iters, stream)
+        torch.cuda.synchronize()      # q and nn are temporaries of this call
+
+    def vertex_areas(self):
+        a = torch.zeros((self.n_cells, self.n_verts), dtype=torch.float32, device=self.device)
+        self.handle.vertex_areas(self.n_cells, self.pos, a)
+        torch.cuda.synchronize()
+        return a.cpu().numpy()
+
     def step_converged(self, tol: float, max_iters: int, stream=None):
         """Converged quasi-Newton step; returns (iterations, residual lengths) per cell (numpy)."""
         its = torch.zeros(self.n_cells, dtype=torch.int32, device=self.device)

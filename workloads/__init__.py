@@ -16,10 +16,12 @@ from .placement import random_rigid_placements, place_cells, quat_to_rot
 from .forces import (gaussian_forces, fourier_shear_field, FourierField, cap_pull_forces,
                      cap_vertex_sets)
 from .configs import CONFIGS, make_config, UNITS
+from .packing import colliding_neighbours, penetration_count, vertex_normals
 
 __all__ = [
     "icosphere", "mesh_counts", "rbc_biconcave", "platelet_ellipsoid", "rest_shape",
     "default_material", "MATERIAL_FIELDS", "random_rigid_placements", "place_cells",
     "quat_to_rot", "gaussian_forces", "fourier_shear_field", "FourierField", "cap_pull_forces",
-    "cap_vertex_sets", "CONFIGS", "make_config", "UNITS",
+    "cap_vertex_sets", "CONFIGS", "make_config", "UNITS", "colliding_neighbours", "penetration_count",
+    "vertex_normals",
 ]

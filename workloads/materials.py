@@ -11,7 +11,7 @@ from .shapes import mesh_volume
 # order of the C struct npfem_material / oracle_material (all doubles)
 MATERIAL_FIELDS = (
     "cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min", "a_max",
-    "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta",
+    "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta", "w_collision", "d_collision",
 )
 
 DENSITY_PG_PER_UM3 = 1.125          # 1125 kg/m^3 (A-4)
