@@ -62,6 +62,9 @@ typedef struct {
   double w_collision;            /* collision weight per vertex (PAPER.md:145 collisions_weight), >= 0; */
   double d_collision;            /* contact distance >= 0: a vertex with a colliding neighbour (q, n)   */
                                  /* is kept at (x - q).n >= d_collision (reading A-22); both 0 = off   */
+  double strain_hardening;       /* beta >= 0: strain-dependent strain weight k_strain (1 + beta d^2),  */
+                                 /* d = clamp(sigma) - sigma (reading A-23: "a weight */
+                                 /* and various parameters ... stiffer or softer"); 0 = constant weight */
 } npfem_material;
 
 /* Tuning knobs that do not change what is computed beyond fp32 rounding.  Pass NULL for defaults. */

@@ -51,6 +51,7 @@ typedef struct {
   double w_volume, v_min, v_max;
   double c_alpha, c_beta;
   double w_collision, d_collision;   /* collision weight per vertex, contact distance (reading A-22) */
+  double strain_hardening;           /* beta >= 0: strain-dependent weight w_s (1 + beta d^2) (reading A-23) */
 } oracle_material;
 
 typedef struct oracle_cell {
@@ -174,6 +175,34 @@ void oracle_project_strain(const double *F, double s_min, double s_max, double *
   d[0] = clampd(S[0], s_min, s_max);
   d[1] = clampd(S[1], s_min, s_max);
   compose32(U, d, V, P);
+}
+
+/* Strain-dependent weight (NEXT-4, reading A-23; "every elemental potential energy
+ * ... has a weight and various parameters", :183 "one can make the material stiffer or softer"):
+ * with d_i = clamp(sigma_i) - sigma_i the strain energy density per singular value becomes
+ *   psi(d) = 1/2 w_s (d^2 + 1/2 beta d^4),   psi'(d) = w_s d (1 + beta d^2),
+ * i.e. the weight grows with the strain, w_s (1 + beta d^2) (hardening).  Following the
+ * quasi-Newton view of projective dynamics (Liu et al.), the local step hands the global step the
+ * EFFECTIVE target  P_eff = F + U diag(d_i (1 + beta d_i^2)) V^T,  so that w_s G^T (P_eff - F)
+ * is the exact elastic force -dPsi/dx, while the system matrix keeps the constant weight w_s. */
+void oracle_project_strain_hardening(const double *F, double s_min, double s_max, double beta, double *P) {
+  double U[6], S[2], V[4], d[2];
+  oracle_svd32(F, U, S, V);
+  for (int i = 0; i < 2; ++i) {
+    double di = clampd(S[i], s_min, s_max) - S[i];
+    d[i] = S[i] + di * (1.0 + beta * di * di);
+  }
+  compose32(U, d, V, P);
+}
+/* strain energy of one triangle per unit weight: 1/2 sum_i (d_i^2 + 1/2 beta d_i^4) */
+double oracle_strain_energy_density(const double *F, double s_min, double s_max, double beta) {
+  double U[6], S[2], V[4], e = 0;
+  oracle_svd32(F, U, S, V);
+  for (int i = 0; i < 2; ++i) {
+    double di = clampd(S[i], s_min, s_max) - S[i];
+    e += 0.5 * (di*di + 0.5 * beta * di*di*di*di);
+  }
+  return e;
 }
 
 /* Closest point (o[0],o[1]) of the hyperbola branch {s1*s2 = a, s > 0} to (sg1,sg2), sg1 >= sg2.
@@ -321,7 +350,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   if (n < 4 || T < 4 || !tris || !X || !mat || !(h > 0)) return ORACLE_EINVAL;
   if (mat->s_min > mat->s_max || mat->a_min > mat->a_max || mat->v_min > mat->v_max) return ORACLE_EINVAL;
   if (mat->c_alpha < 0.0 || mat->c_beta < 0.0) return ORACLE_EINVAL;
-  if (mat->w_collision < 0.0 || mat->d_collision < 0.0) return ORACLE_EINVAL;
+  if (mat->w_collision < 0.0 || mat->d_collision < 0.0 || mat->strain_hardening < 0.0) return ORACLE_EINVAL;
   if (!(mat->cell_mass > 0)) return ORACLE_EINVAL;
   for (int i = 0; i < 3*T; ++i) if (tris[i] < 0 || tris[i] >= n) return ORACLE_EINVAL;
   if ((3*T) % 2) return ORACLE_EINVAL;
@@ -486,7 +515,8 @@ void oracle_local(const oracle_cell *c, const double *x, double *Ps, double *Pa,
   for (int t = 0; t < c->T; ++t) {
     double F[6];
     oracle_deformation_gradient(c, t, x, F);
-    oracle_project_strain(F, m->s_min, m->s_max, Ps + 6*t);
+    if (m->strain_hardening != 0.0) oracle_project_strain_hardening(F, m->s_min, m->s_max, m->strain_hardening, Ps + 6*t);
+    else oracle_project_strain(F, m->s_min, m->s_max, Ps + 6*t);
     oracle_project_area(F, m->a_min, m->a_max, Pa + 6*t);
   }
   for (int hh = 0; hh < c->H; ++hh) {
@@ -561,7 +591,10 @@ double oracle_energy(const oracle_cell *c, const double *x, const double *s, con
       ds += (F[k]-Ps[6*t+k])*(F[k]-Ps[6*t+k]);
       da += (F[k]-Pa[6*t+k])*(F[k]-Pa[6*t+k]);
     }
-    e[1] += 0.5 * m->k_strain * c->area[t] * ds;
+    if (m->strain_hardening != 0.0)      /* Ps holds the effective targets: take the energy from F itself */
+      e[1] += m->k_strain * c->area[t] * oracle_strain_energy_density(F, m->s_min, m->s_max, m->strain_hardening);
+    else
+      e[1] += 0.5 * m->k_strain * c->area[t] * ds;
     e[2] += 0.5 * m->k_area * c->area[t] * da;
   }
   for (int hh = 0; hh < c->H; ++hh) {

@@ -16,7 +16,7 @@ from . import build as _build
 
 MATERIAL_FIELDS = ("cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min", "a_max",
                    "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta", "w_collision",
-                   "d_collision")
+                   "d_collision", "strain_hardening")
 
 
 class _Material(C.Structure):

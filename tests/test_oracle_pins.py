@@ -754,3 +754,42 @@ def test_P25_vertex_areas():
     sph, st = W.mesh.icosphere(3)
     cs = O.OracleCell(st, sph, W.default_material(sph, st), DT)
     assert 0.98 * 4 * np.pi < cs.vertex_areas(sph).sum() < 4 * np.pi
+
+
+# ----------------------------------------------------------------------------- strain-dependent weight (A-23)
+def test_P26_strain_hardening_energy_force_and_fixed_point():
+    """psi(d) = 1/2 w_s (d^2 + 1/2 beta d^4): (i) closed form under uniform scaling,
+    E_strain = k_strain A_tot ((s-1)^2 + 1/2 beta (s-1)^4); (ii) f_int = -grad E by central
+    differences (the effective targets carry psi'); (iii) the rest shape is still a fixed point and
+    beta = 0 is the plain strain term; (iv) hardening stiffens: smaller stretch under the same pull."""
+    beta = 40.0
+    c, rest, tris, mat = make_cell("rbc", 2, strain_hardening=beta)
+    c0, _, _, _ = make_cell("rbc", 2)
+    a_tot = c.areas().sum()
+    for sc in (0.9, 1.1, 1.3):
+        x = rest * sc
+        _, parts = c.energy(x, x, c.local(x), parts=True)
+        assert parts[1] == pytest.approx(mat["k_strain"] * a_tot * ((sc - 1) ** 2 + 0.5 * beta * (sc - 1) ** 4), rel=1e-9)
+    rng = np.random.default_rng(61)
+    x = rest * 1.08 + 0.02 * rng.standard_normal(rest.shape)
+    f = c.fint(x)
+
+    def E(y):
+        _, parts = c.energy(y, y, c.local(y), parts=True)
+        return parts[1:].sum()
+
+    eps = 1e-6
+    for _ in range(10):
+        i, d = rng.integers(rest.shape[0]), rng.integers(3)
+        e = np.zeros_like(x); e[i, d] = eps
+        assert -(E(x + e) - E(x - e)) / (2 * eps) == pytest.approx(f[i, d], rel=2e-5, abs=1e-9)
+    assert np.abs(f - c0.fint(x)).max() > 1e-3 * np.abs(f).max()         # and it differs from beta = 0
+    z = np.zeros_like(rest)
+    xr, vr = c.step_cell(rest, z, z, 10)
+    assert np.abs(xr - rest).max() < 1e-13
+    pull = W.cap_pull_forces(rest, np.eye(3)[None], 40e-3)[0].astype(np.float64)
+    xs, vs, xh, vh = rest.copy(), z.copy(), rest.copy(), z.copy()
+    for _ in range(150):
+        xs, vs = c0.step_cell(xs, vs, pull, 10)
+        xh, vh = c.step_cell(xh, vh, pull, 10)
+    assert np.ptp(xh[:, 0]) < np.ptp(xs[:, 0]) - 1e-3

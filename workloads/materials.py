@@ -12,6 +12,7 @@ from .shapes import mesh_volume
 MATERIAL_FIELDS = (
     "cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min", "a_max",
     "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta", "w_collision", "d_collision",
+    "strain_hardening",
 )
 
 DENSITY_PG_PER_UM3 = 1.125          # 1125 kg/m^3 (A-4)
@@ -27,6 +28,7 @@ def default_material(rest_xyz, tris, **overrides) -> dict:
         w_volume=0.5, v_min=1.0, v_max=1.0,
         c_alpha=0.0, c_beta=0.0,
         w_collision=0.0, d_collision=0.0,
+        strain_hardening=0.0,
     )
     for k, v in overrides.items():
         if k not in mat:
