@@ -322,6 +322,7 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.jitter = P.opt.debug_jitter;
   D.coll_q = nullptr; D.coll_n = nullptr;
   D.w_coll = (float)P.mat.w_collision; D.d_coll = (float)P.mat.d_collision;
+  D.hard = (float)P.mat.strain_hardening;
   D.L = smem_layout(n, E, P.nvb, P.cells_per_cta);
   if (max_cells > 0) {   // everything any later step entry point needs exists now
     rc = create_pipeline(H, max_cells);

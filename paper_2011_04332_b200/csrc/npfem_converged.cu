@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_converged_kernel(const DevParam
   // ---- f_int and E_el at the iterate in z4: element pass, vertex gather, volume projection.
   //      Returns this vertex's elastic residual ev and its share en of g (inertial term included).
   auto evaluate = [&](F3 zv, F3& ev, float& en) {
-    if (is_e) element_residual<3>(ecs + tid, E, z4b, P, reinterpret_cast<float4*>(rbb) + tid);
+    if (is_e) element_residual<3, true>(ecs + tid, E, z4b, P, reinterpret_cast<float4*>(rbb) + tid);
     const uint4 vr0 = P.vrole[2 * v];
     const uint4 vr1 = P.vrole[2 * v + 1];
     const int icnt = vr0.w & 0xff, rcnt = (vr0.w >> 8) & 0xff;

@@ -123,7 +123,8 @@ __device__ __forceinline__ float hyperbola_p(float s1, float s2, float q, float 
 // once per step on y = x_n - c to form the constant part of the damping force).
 // KIND 3: residual as KIND 0, and the triangle's energy 1/2 w_s dist^2(F, strain set) +
 // 1/2 w_a dist^2(F, area set) is added to `en` (converged solve: the line search needs g).
-template <int KIND>
+// HARD: strain-dependent strain weight w_s (1 + beta d^2) (reading A-23), beta = P.hard at run time.
+template <int KIND, bool HARD>
 __device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, float i11, float ws,
                                          float wa, const DevParams& P, F3& f1, F3& f2, float& en) {
   if (KIND == 2) {
@@ -150,7 +151,14 @@ __device__ __forceinline__ void membrane(F3 e1, F3 e2, float i00, float i01, flo
   const float d1 = fminf(fmaxf(s1, P.s_min), P.s_max) - s1, d2 = fminf(fmaxf(s2, P.s_min), P.s_max) - s2;
   float g1 = ws * d1 * r1;
   float g2 = ws * d2 * r2;
-  if (KIND == 3) en = fmaf(0.5f * ws, fmaf(d1, d1, d2 * d2), en);
+  if (HARD) {
+    g1 *= fmaf(P.hard, d1 * d1, 1.0f);
+    g2 *= fmaf(P.hard, d2 * d2, 1.0f);
+  }
+  if (KIND == 3) {
+    const float q1 = d1 * d1, q2 = d2 * d2;
+    en = fmaf(0.5f * ws, HARD ? fmaf(0.5f * P.hard, fmaf(q1, q1, q2 * q2), q1 + q2) : q1 + q2, en);
+  }
   const float astar = fminf(fmaxf(J, P.a_min), P.a_max);
   if (J != astar) {
     const float q = fsqrt(astar);
@@ -237,7 +245,7 @@ __device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
 // Local step of one element for one cell: membrane residuals of its two triangles and the five
 // hinges it sees, summed per own vertex (a,b,c,d) into out4[slot * E].  ec = the element's
 // constants in shared memory (group g at ec[g * E], npfem_api.cu), zc = the cell's z4 array.
-template <int KIND>
+template <int KIND, bool HARD = false>
 __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, int E,
                                                  const unsigned char* __restrict__ zc,
                                                  const DevParams& P, float4* __restrict__ out4) {
@@ -293,8 +301,8 @@ __device__ __forceinline__ void element_residual(const float4* __restrict__ ec, 
   {
     const float4 m1 = ec[E], m2 = ec[2 * E];
     F3 t1b, t1c, t2a, t2d;
-    membrane<KIND>(eab, eac, m1.x, m1.y, m1.z, m1.w, m3.x, P, t1b, t1c, en);
-    membrane<KIND>(eba, ebd, m2.x, m2.y, m2.z, m2.w, m3.y, P, t2a, t2d, en);
+    membrane<KIND, HARD>(eab, eac, m1.x, m1.y, m1.z, m1.w, m3.x, P, t1b, t1c, en);
+    membrane<KIND, HARD>(eba, ebd, m2.x, m2.y, m2.z, m2.w, m3.y, P, t2a, t2d, en);
     fa = fa + (t2a - (t1b + t1c));
     fb = fb + (t1b - (t2a + t2d));
     fc = fc + t1c;

@@ -50,7 +50,8 @@ __device__ __forceinline__ void jitter_sleep(int seed, int phase, int warp) {
 // mma.sync on the block-sparse inverse.
 // ------------------------------------------------------------------------------------------
 // FEAT 0: the lean kernel of the headline path; FEAT 1: damping (compile-time) plus the run-time
-// options; FEAT 2: undamped with the run-time options (collision neighbours, debug_jitter).
+// options; FEAT 2: undamped with the run-time options (collision neighbours, strain hardening,
+// debug_jitter).
 template <int MODE, int MAXT, int FEAT>
 __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) {
   constexpr bool DAMP = FEAT == 1, OPT = FEAT != 0;
@@ -225,7 +226,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     // so the vertex phase of cell c and the element pass of cell c+1 share one barrier interval
     auto elements_and_gradient = [&](int cc) {
       const unsigned char* zcc = z4b + cc * cellz;
-      if (is_e) element_residual<DAMP ? 1 : 0>(ec_t, E, zcc, P, reinterpret_cast<float4*>((cc & 1) ? rab : rbb) + tid);
+      if (is_e) element_residual<DAMP ? 1 : 0, OPT>(ec_t, E, zcc, P, reinterpret_cast<float4*>((cc & 1) ? rab : rbb) + tid);
       vr0 = P.vrole[2 * v];
       if (use_vol) {
         float S1 = 0.f, S2 = 0.f;
@@ -517,7 +518,7 @@ cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mod
                         cudaStream_t stream) {
   if (p.n_cells <= 0) return cudaSuccess;
   const int grid = (p.n_cells + p.k - 1) / p.k;
-  const int feat = p.damped ? 1 : (p.coll_n != nullptr || p.jitter != 0) ? 2 : 0;
+  const int feat = p.damped ? 1 : (p.coll_n != nullptr || p.jitter != 0 || p.hard != 0.0f) ? 2 : 0;
 #define NPFEM_LAUNCH(MODE, MAXT)                                                                  \
   do {                                                                                            \
     if (feat == 1) npfem_step_kernel<MODE, MAXT, 1><<<grid, threads, smem_bytes, stream>>>(p);    \

@@ -41,6 +41,7 @@ struct DevParams {
   const float* coll_q;                     // [n_cells][cell_stride] colliding neighbour point per vertex, or NULL
   const float* coll_n;                     // [n_cells][cell_stride] its outward unit normal (0 = none), or NULL
   float w_coll, d_coll;                    // collision weight, contact distance (A-22)
+  float hard;                              // strain hardening beta (A-23)
   SmemLayout L;
 };
 

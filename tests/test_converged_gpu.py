@@ -117,3 +117,27 @@ def test_large_time_step_converged_vs_fixed_sweeps():
     print(f"[converged] dt x 10: residual after 20 fixed sweeps {out['fixed']:.2e}, converged {out['converged']:.2e} "
           f"in {its.tolist()} iterations")
     assert out["converged"] <= 2 * TOL[10] and out["fixed"] > 20 * out["converged"]
+
+
+def test_converged_step_with_strain_dependent_weight():
+    """The converged solve minimises the true (non-quadratic) energy when k_strain depends on the
+    strain (A-23): same minimiser as the oracle's L-BFGS at 10 dt."""
+    dt = 1.0
+    rest, tris = W.rest_shape("rbc", 2)
+    mat = W.default_material(rest, tris, strain_hardening=60.0)
+    rng = np.random.Generator(np.random.PCG64([91, 7]))
+    rot, trans = W.random_rigid_placements(4, 100.0, 5.0, rng)
+    pos0 = W.place_cells(rest * 1.04, rot, trans)
+    vel0 = np.zeros_like(pos0)
+    f = W.gaussian_forces(pos0.shape, 5e-3, 91, 0)
+    dg = DeviceGroup(tris, rest, mat, dt, pos0, vel0)
+    dg.set_forces(f)
+    its, res = dg.step_converged(TOL[10], 1000)
+    pg, vg = dg.state()
+    oc = O.OracleCell(tris, rest, mat, dt)
+    po, vo, its_o = oc.step_converged(pos0, vel0, f, TOL[10] / 20, 3000, history=3)
+    for c in range(4):
+        assert its[c] < 1000 and res[c] <= TOL[10]
+        xn = pos0[c].astype(np.float64)
+        dx_o = po[c] - xn
+        assert np.abs(xn + vg[c].astype(np.float64) * dt - po[c]).max() <= 1e-3 * np.abs(dx_o).max() + 2 * TOL[10]

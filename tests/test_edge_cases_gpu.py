@@ -289,3 +289,23 @@ def test_schedule_jitter_leaves_results_bit_identical():
         for seed in (1, 2, 3):
             out = list(gpu_trajectory(g, 0.1, forces[:2], 6, debug_jitter=seed, **opt))[-1]
             assert np.array_equal(ref[0], out[0]) and np.array_equal(ref[1], out[1]), (name, seed)
+
+
+@pytest.mark.parametrize("damp", [{}, dict(c_alpha=0.3, c_beta=0.02)])
+def test_strain_dependent_weight_matches_the_oracle(damp):
+    """NEXT-4 (reading A-23): strain weight k_strain (1 + beta d^2).  Forces large
+    enough to strain the membrane by several per cent, so that the hardening factor really differs
+    from 1; with and without damping (both optioned kernel instantiations)."""
+    rest, tris, mat, pos0, vel0, forces = _small_workload(n_cells=6, sigma=2e-2, strain_hardening=60.0, **damp)
+    g = _G(rest, tris, mat, pos0, vel0)
+    forces = list(forces) * 3                                     # 9 steps
+    _parity(g, forces, 12)
+    oc = O.OracleCell(tris, rest, mat, 0.1)
+    last = list(oracle_trajectory(g, 0.1, forces, 12))[-1][0][0]
+    sv = np.array([np.linalg.svd(oc.deformation_gradient(t, last), compute_uv=False) for t in range(tris.shape[0])])
+    assert np.abs(sv - 1).max() > 0.03                            # beta d^2 > 5 % somewhere
+    # and it is not a no-op
+    a = list(gpu_trajectory(g, 0.1, forces, 12))[-1][0]
+    g0 = _G(rest, tris, W.default_material(rest, tris, **damp), pos0, vel0)
+    b = list(gpu_trajectory(g0, 0.1, forces, 12))[-1][0]
+    assert np.abs(a.astype(np.float64) - b).max() > 1e-4
