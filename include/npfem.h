@@ -78,7 +78,10 @@ typedef struct {
                           /* it cannot change the result at fp32 resolution (A-17), so    */
                           /* near-rest cells take one pass whatever the cap                         */
   int cells_per_cta;      /* 1..5 cells share one CTA and every fetched operator block; 0 = auto   */
-  int global_mode;        /* 0 = auto, 1 = fp32 SIMT blocks, 2 = 3xTF32 tensor-core blocks          */
+  int global_mode;        /* 0 = auto (3 where it applies, else 2), 1 = fp32 SIMT blocks,           */
+                          /* 2 = 3xTF32 tensor-core blocks, 3 = two-term fp16 split (hi*hi + hi*lo  */
+                          /* + lo*hi, fp32 accumulate; like 3xTF32 exact to fp32 rounding) on       */
+                          /* mma.m16n8k16, two blocks per product, per-warp operator streams        */
   int pair_triangles;     /* local-step work items: 0 = auto / 1 = pairs of triangles across a shared */
                           /* edge wherever the matching finds one, 2 = one triangle per item        */
   int debug_jitter;       /* 0 = off; otherwise a seed: every warp of the step kernel sleeps a      */
@@ -203,6 +206,16 @@ int npfem_cell_stride(npfem_handle h); /* floats per cell actually used         
  */
 int npfem_measure_fp32_peak(int variant, double* out_tflops);
 
+/*
+ * npfem_debug_phase_clocks: diagnostic builds only (nvcc -DNPFEM_PHASE_CLOCKS; the shipped library
+ * returns NPFEM_EINVAL).  Copies 16 counters of clock64() ticks that thread 0 of every CTA of the
+ * step kernel accumulates per phase of an iteration (0 prologue, 1 first element pass, 2 cell
+ * pipeline, 3 right-hand-side split, 4 operator product, 5 hand-off, 6 owner update), summed over
+ * CTAs and iterations since the last reset.  Blocking.
+ *   out16  host, receives 16 counters;  reset  non-zero: zero the counters after reading
+ */
+int npfem_debug_phase_clocks(unsigned long long* out16, int reset);
+
 /* Introspection of a handle (all host-side, cheap): what the create step decided.               */
 typedef struct {
   int n_verts, n_tris, n_hinges;
@@ -213,13 +226,15 @@ typedef struct {
   int n_vblocks;       /* ceil(n_verts/8): operator is stored as 8x8 blocks */
   int n_op_blocks;     /* kept 8x8 blocks of A_sys^-1 */
   int op_nnz;          /* entries of A_sys^-1 kept by the drop rule (before blocking) */
-  int global_mode;     /* 1 = SIMT, 2 = 3xTF32 */
+  int global_mode;     /* 1 = SIMT, 2 = 3xTF32, 3 = two-term fp16 split */
   int volume_inner_iters;
   int n_op_blocks_tf32x1; /* of n_op_blocks, blocks applied as ONE TF32 product: their share of   */
                           /* every row's l1 mass is <= 2^-15, so the product error stays below   */
                           /* fp32 rounding of the row sum; all other blocks use 3xTF32            */
   int n_elements;         /* threads' work items of the local step: pairs of triangles sharing an  */
   int n_diamonds;         /* edge (n_diamonds of them) plus triangles left single by the matching  */
+  int n_op_blocks_f16x1;  /* global_mode 3: of n_op_blocks, blocks applied as ONE fp16 product (hi   */
+                          /* parts only): their share of every row's l1 mass is <= 2^-13            */
   double rest_volume, total_mass, inv_drop_tol;
 } npfem_info;
 int npfem_get_info(npfem_handle h, npfem_info* out);
@@ -247,6 +262,10 @@ int npfem_plan_info(npfem_plan p, npfem_info* out);
 #define NPFEM_Q_TRI_AREA 9    /* double [n_tris]                                                   */
 #define NPFEM_Q_OPERATOR_X1 10 /* double [n_verts^2]: like NPFEM_Q_OPERATOR, only the blocks that are    */
                               /* applied as one TF32 product (npfem_info.n_op_blocks_tf32x1)       */
+#define NPFEM_Q_OPERATOR_F16 11 /* double [n_verts^2]: the global_mode-3 operator (hi + lo fp16 parts,  */
+                              /* row scaling undone) expanded to a dense matrix in caller order;   */
+                              /* one-product blocks contribute their hi part only                  */
+#define NPFEM_Q_OPERATOR_F16X1 12 /* double [n_verts^2]: only the blocks applied as one fp16 product */
 int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems);
 
 #ifdef __cplusplus

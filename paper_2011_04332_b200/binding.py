@@ -19,7 +19,8 @@ MATERIAL_FIELDS = ("cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min",
 QUERY = {"perm": (1, np.int32), "mass": (2, np.float64), "system": (3, np.float64),
          "operator": (4, np.float64), "hinge_verts": (5, np.int32), "hinge_K": (6, np.float64),
          "hinge_wr": (7, np.float64), "tri_dminv": (8, np.float64), "tri_area": (9, np.float64),
-         "operator_x1": (10, np.float64)}
+         "operator_x1": (10, np.float64), "operator_f16": (11, np.float64),
+         "operator_f16x1": (12, np.float64)}
 
 ERROR_NAMES = {0: "NPFEM_OK", -1: "NPFEM_EINVAL", -2: "NPFEM_ENOMEM", -3: "NPFEM_ECUDA",
                -4: "NPFEM_ELIMIT"}
@@ -39,7 +40,7 @@ class Info(C.Structure):
     _fields_ = [(f, C.c_int) for f in (
         "n_verts", "n_tris", "n_hinges", "cell_stride", "cells_per_cta", "threads_per_cta",
         "smem_bytes", "n_vblocks", "n_op_blocks", "op_nnz", "global_mode",
-        "volume_inner_iters", "n_op_blocks_tf32x1", "n_elements", "n_diamonds")] + [(f, C.c_double) for f in ("rest_volume", "total_mass",
+        "volume_inner_iters", "n_op_blocks_tf32x1", "n_elements", "n_diamonds", "n_op_blocks_f16x1")] + [(f, C.c_double) for f in ("rest_volume", "total_mass",
                                                             "inv_drop_tol")]
 
     def as_dict(self) -> dict:
@@ -94,6 +95,8 @@ def load_library(path: str | None = None):
     lib.npfem_plan_query.argtypes = [vp, C.c_int, vp, C.c_int]
     lib.npfem_measure_fp32_peak.restype = C.c_int
     lib.npfem_measure_fp32_peak.argtypes = [C.c_int, dp]
+    lib.npfem_debug_phase_clocks.restype = C.c_int
+    lib.npfem_debug_phase_clocks.argtypes = [C.POINTER(C.c_ulonglong), C.c_int]
     if path is None:
         _lib = lib
     return lib
@@ -104,6 +107,13 @@ def npfem_measure_fp32_peak(variant: int = 0) -> float:
     out = C.c_double(0.0)
     _check(load_library().npfem_measure_fp32_peak(int(variant), C.byref(out)))
     return float(out.value)
+
+
+def npfem_debug_phase_clocks(reset: bool = True) -> list:
+    """Diagnostic builds only (-DNPFEM_PHASE_CLOCKS): the 16 per-phase tick counters of the step kernel."""
+    out = (C.c_ulonglong * 16)()
+    _check(load_library().npfem_debug_phase_clocks(out, int(reset)))
+    return [int(x) for x in out]
 
 
 def npfem_last_error() -> str:

@@ -40,6 +40,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
            "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
            "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    extra = os.environ.get("NPFEM_NVCC_FLAGS", "")   # diagnostic builds, e.g. -DNPFEM_PHASE_CLOCKS
+    if extra:
+        cmd += extra.split()
     if verbose:
         cmd += ["-Xptxas", "-v"]
     subprocess.run(cmd, check=True)

@@ -3,6 +3,7 @@
 // math: npfem_plan.cpp; step math: npfem_kernels.cu).
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -56,6 +57,7 @@ void fill_info(const Plan& P, int cell_stride, npfem_info* o) {
   o->n_op_blocks_tf32x1 = P.n_op_blocks_x1;
   o->n_elements = P.E;
   o->n_diamonds = P.n_diamonds;
+  o->n_op_blocks_f16x1 = P.n_op_blocks_h1;
   o->op_nnz = P.op_nnz;
   o->global_mode = P.global_mode;
   o->volume_inner_iters = P.opt.volume_inner_iters;
@@ -198,6 +200,40 @@ int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems) {
         }
       return (int)elems;
     }
+    case NPFEM_Q_OPERATOR_F16:
+    case NPFEM_Q_OPERATOR_F16X1: {
+      const size_t elems = (size_t)n * n;
+      if (!dst) return (int)elems;
+      if ((size_t)dst_elems < elems) return set_err(NPFEM_EINVAL, "destination too small");
+      double* D = static_cast<double*>(dst);
+      std::memset(D, 0, elems * sizeof(double));
+      auto hv = [](uint32_t w, int q) {   // value of half q of a packed word
+        const uint32_t hb = (w >> (16 * q)) & 0xffffu;
+        const int e = (hb >> 10) & 0x1f, m = hb & 0x3ff;
+        const double v = e == 0 ? std::ldexp((double)m, -24) : std::ldexp((double)(m | 0x400), e - 25);
+        return (hb & 0x8000u) ? -v : v;
+      };
+      for (int ib = 0; ib < P.nvb; ++ib)
+        for (int pass = (what == NPFEM_Q_OPERATOR_F16X1 ? 1 : 0); pass < 2; ++pass) {
+          const std::vector<uint32_t>& col = pass ? P.hp_col_b : P.hp_col_a;
+          const std::vector<uint32_t>& val = pass ? P.hp_val_b : P.hp_val_a;
+          const int words = pass ? 2 : 4;
+          for (int pr = P.hp_ptr[4 * ib + 2 * pass]; pr < P.hp_ptr[4 * ib + 2 * pass + 1]; ++pr)
+            for (int l = 0; l < 32; ++l)
+              for (int half = 0; half < 2; ++half) {
+                const int jb = (int)((col[pr] >> (16 * half)) & 0xffffu);
+                if (jb == 0xffff) continue;
+                for (int q = 0; q < 2; ++q) {
+                  const int i = ib * 8 + (l >> 2), j = jb * 8 + 2 * (l & 3) + q;
+                  if (i >= n || j >= n) continue;
+                  double x = hv(val[((size_t)pr * 32 + l) * words + half], q);
+                  if (!pass) x += hv(val[((size_t)pr * 32 + l) * words + 2 + half], q);
+                  D[(size_t)P.perm[i] * n + P.perm[j]] += x * (double)P.hp_scale[i];
+                }
+              }
+        }
+      return (int)elems;
+    }
     default: return set_err(NPFEM_EINVAL, "unknown query");
   }
 }
@@ -243,12 +279,13 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   //   0: packed byte offsets 16*id of (a,b) (c,d) (f1,f2) (f3,f4)   1: t1 i00 i01 i11 w_s
   //   2: t2 i00 i01 i11 w_s      3: t1 w_a, t2 w_a, he, 0           4..8: hinge e: Kp Kq Ko r'
   std::vector<uint32_t> elem_c((size_t)kElemGroups * E * 4, 0u);
-  std::vector<float> h2m(NP, 0.0f), mh2(NP, 0.0f), dmp(NP, 0.0f);
+  std::vector<float> h2m(NP, 0.0f), mh2(NP, 0.0f), dmp(NP, 0.0f), hps(NP, 0.0f);
   for (int i = 0; i < n; ++i) {
     perm16[i] = (uint16_t)P.perm[i];
     h2m[i] = P.h2_over_m[i];
     mh2[i] = P.m_over_h2[i];
     dmp[i] = P.damp_m[i];
+    hps[i] = P.hp_scale[i];
   }
   auto fbits = [](float x) { uint32_t u; std::memcpy(&u, &x, 4); return u; };
   for (int e = 0; e < E; ++e) {
@@ -286,6 +323,8 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
       {P.ring_off.data(), P.ring_off.size() * 2, 0},  {P.blk_ptr.data(), P.blk_ptr.size() * 4, 0},
       {P.blk_col.data(), P.blk_col.size() * 2, 0},    {P.blk_val.data(), P.blk_val.size() * 4, 0},
       {dmp.data(), dmp.size() * 4, 0},
+      {P.hs_val.data(), P.hs_val.size() * 4, 0},      {hps.data(), hps.size() * 4, 0},
+      {P.hs_desc.data(), P.hs_desc.size() * 4, 0},
   };
   size_t total = 0;
   for (auto& sct : secs) { sct.off = total; total += align_up(sct.bytes, 256); }
@@ -317,9 +356,16 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
   D.blk_col = reinterpret_cast<const uint16_t*>(base + secs[10].off);
   D.blk_val = reinterpret_cast<const float*>(base + secs[11].off);
   D.damp_m = reinterpret_cast<const float*>(base + secs[12].off);
+  D.hs_val = reinterpret_cast<const uint4*>(base + secs[13].off);
+  D.hp_scale = reinterpret_cast<const float*>(base + secs[14].off);
+  D.hs_desc = reinterpret_cast<const uint4*>(base + secs[15].off);
+  D.hs_slots = P.hs_slots;
+  for (int j = 0; j < 4; ++j) { D.hs_na[j] = P.hs_na[j]; D.hs_nb[j] = P.hs_nb[j]; }
+  std::memcpy(D.hs_rows, P.hs_rows.data(), sizeof(D.hs_rows));
   D.cbh = (float)(P.mat.c_beta / P.h);
   D.damped = P.damped ? 1 : 0;
   D.jitter = P.opt.debug_jitter;
+  D.dbg = 0;
   D.coll_q = nullptr; D.coll_n = nullptr;
   D.w_coll = (float)P.mat.w_collision; D.d_coll = (float)P.mat.d_collision;
   D.hard = (float)P.mat.strain_hardening;
@@ -329,6 +375,14 @@ int npfem_create(int n_verts, int n_tris, const int32_t* tris, const double* res
     if (rc != NPFEM_OK) { cudaFree(H->blob); delete H; return rc; }
   }
   *out = H;
+  return NPFEM_OK;
+}
+
+int npfem_debug_phase_clocks(unsigned long long* out16, int reset) {
+  if (!out16) return set_err(NPFEM_EINVAL, "null argument");
+  cudaError_t e = read_phase_clocks(out16, reset);
+  if (e == cudaErrorNotSupported) return set_err(NPFEM_EINVAL, "library built without -DNPFEM_PHASE_CLOCKS");
+  if (e != cudaSuccess) return cuda_err(e, "npfem_debug_phase_clocks");
   return NPFEM_OK;
 }
 

@@ -11,6 +11,14 @@
 namespace npfem {
 namespace {
 
+// Diagnostic builds (-DNPFEM_PHASE_CLOCKS): ablation mask of the MODE 3 operator product, a kernel
+// parameter (DevParams::dbg): 1 no mma, 2 no shared loads, 4 no stream loads, 8 no descriptor loads.
+#ifdef NPFEM_PHASE_CLOCKS
+#define NPFEM_DBG(bit) (dbg & (bit))
+#else
+#define NPFEM_DBG(bit) 0
+#endif
+
 struct F3 {
   float x, y, z;
 };
@@ -210,10 +218,33 @@ __device__ __forceinline__ void mma_tf32(float (&c)[4], const uint32_t (&a)[4], 
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
 }
 
+// global_mode 3: D(16 rhs columns x 8 output vertices) += A(16 x 16 fp16) B(16 x 8 fp16), fp32 accumulate
+__device__ __forceinline__ void mma_f16(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                        uint32_t b0, uint32_t b1, int dbg = 0) {
+  if (NPFEM_DBG(1)) { c[0] += __uint_as_float(a0 ^ b0); c[1] += __uint_as_float(a1 ^ b1); c[2] += __uint_as_float(a2); c[3] += __uint_as_float(a3); return; }
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, "
+      "{%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
 // Operator blocks stream from L2 once per use: keep them out of L1, which holds the register spills.
 __device__ __forceinline__ float2 ldg_stream(const float2* p) {
   float2 v;
   asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  return v;
+}
+
+__device__ __forceinline__ uint4 ldg_stream(const uint4* p) {
+  uint4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint2 ldg_stream(const uint2* p) {
+  uint2 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
   return v;
 }
 
@@ -231,6 +262,11 @@ __device__ __forceinline__ void tmem_st4(uint32_t a, float v0, float v1, float v
   asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
                :: "r"(a), "f"(v0), "f"(v1), "f"(v2), "f"(v3) : "memory");
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t a, float& v0, float& v1, float& v2, float& v3) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+               : "=f"(v0), "=f"(v1), "=f"(v2), "=f"(v3) : "r"(a) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void tmem_ld16(uint32_t a, float (&v)[16]) {
   asm volatile(
@@ -403,6 +439,37 @@ __device__ __forceinline__ void block_run(float (&acc)[4], float (&accx)[4], con
       }
     }
   }
+}
+
+// global_mode 3: the products of one slot of a warp's operator stream (npfem_internal.h).  A pair
+// = two source blocks = K = 16 of one mma.m16n8k16; the A fragment halves come from the right-hand
+// sides in shared memory: source block kb sits at A + 512 kb, hi plane then (256 bytes further) lo
+// plane, each 32 chunks of 8 bytes {col g, col g+8} x vertices (2t, 2t+1), chunk index
+// (4 g + t) ^ 4 (kb & 7) (bank swizzle of the split pass), so a lane's address is lane8 ^ the
+// descriptor's half word.  Three-product slot: hi*hi -> acc, lo*hi + hi*lo -> accx.
+__device__ __forceinline__ uint2 lds64(const unsigned char* p) { return *reinterpret_cast<const uint2*>(p); }
+__device__ __forceinline__ void slot_mma3(float (&acc)[4], float (&accx)[4], uint4 b, uint32_t w,
+                                          const unsigned char* A, uint32_t lane8, int dbg = 0) {
+  const unsigned char* A1 = A + ((w & 0xffffu) ^ lane8);
+  const unsigned char* A2 = A + ((w >> 16) ^ lane8);
+  uint2 h1, h2, l1, l2;
+  if (NPFEM_DBG(2)) { h1 = make_uint2(w, lane8); h2 = h1; l1 = h1; l2 = h1; }
+  else { h1 = lds64(A1); h2 = lds64(A2); l1 = lds64(A1 + 256); l2 = lds64(A2 + 256); }
+  mma_f16(accx, l1.x, l1.y, l2.x, l2.y, b.x, b.y, dbg);
+  mma_f16(accx, h1.x, h1.y, h2.x, h2.y, b.z, b.w, dbg);
+  mma_f16(acc, h1.x, h1.y, h2.x, h2.y, b.x, b.y, dbg);
+}
+// One-product slot: two pairs, hi*hi each, one per accumulator chain.
+__device__ __forceinline__ void slot_mma1(float (&acc)[4], float (&accx)[4], uint4 b, uint2 d,
+                                          const unsigned char* A, uint32_t lane8, int dbg = 0) {
+  uint2 h1, h2, h3, h4;
+  if (NPFEM_DBG(2)) { h1 = make_uint2(d.x, lane8); h2 = h1; h3 = h1; h4 = h1; }
+  else {
+    h1 = lds64(A + ((d.x & 0xffffu) ^ lane8)); h2 = lds64(A + ((d.x >> 16) ^ lane8));
+    h3 = lds64(A + ((d.y & 0xffffu) ^ lane8)); h4 = lds64(A + ((d.y >> 16) ^ lane8));
+  }
+  mma_f16(acc, h1.x, h1.y, h2.x, h2.y, b.x, b.y, dbg);
+  mma_f16(accx, h3.x, h3.y, h4.x, h4.y, b.z, b.w, dbg);
 }
 
 }  // namespace

@@ -15,6 +15,7 @@ constexpr int kMaxCellsPerCta = 5;    // 5 cells x 3 coordinates = 15 right-hand
 constexpr int kRhs = 16;              // right-hand sides per CTA in the global step (mma M)
 constexpr int kElemFloats = 31;       // per-element float constants (see ElemConst below)
 constexpr int kRegList = 6;           // incidence / ring entries a vertex thread keeps in registers
+constexpr int kMaxOpSlots = 64;       // global_mode 3: slots per warp whose descriptors fit four registers per lane
 constexpr int kSmemMaxDynamic = 232448 - 1024;   // 227 KB opt-in limit per CTA minus static shared memory
 
 // One ELEMENT = the work of one thread in the local step: a "diamond" of two triangles
@@ -73,6 +74,33 @@ struct Plan {
   std::vector<int32_t> blk_ptr;      // [nvb][3] per OUTPUT block row: first 3xTF32 block, first 1xTF32 block, end
   std::vector<uint16_t> blk_col;     // [n_blocks_padded] source block index
   std::vector<float> blk_val;        // [n_blocks_padded][64] in mma B-fragment order
+  // The same operator for global_mode 3 (two-term fp16 split, mma m16n8k16): the kept blocks of an
+  // OUTPUT block row grouped in PAIRS of source blocks (one mma covers K = 16 = two source blocks):
+  // first the pairs applied with three products (hi*hi + hi*lo + lo*hi), then the pairs whose
+  // blocks are so small that the hi*hi product alone is exact to fp32 rounding of the row sum.
+  // Rows are scaled by a power of two (hp_scale) so that their entries sit in the fp16 range.
+  // Every warp of the step kernel owns up to 4 output block rows ("row slots" j = 0..3) and consumes
+  // ONE contiguous stream of 512-byte SLOTS (16 bytes per lane) in a fixed order that is the same
+  // for all warps: per row slot j first hs_na[j] three-product slots (one pair each: B fragment hi,
+  // lo), then hs_nb[j] one-product slots (two pairs each: hi, hi).  Rows are sorted by cost and
+  // dealt to the row slots so that the rows of a slot have similar lengths; shorter rows are padded
+  // with zero pairs (the phase ends at a CTA barrier, so the longest row of a slot sets the time
+  // anyway).  Uniform shapes make every branch of the product loop warp-uniform at compile time.
+  // A slot's descriptor holds the byte offsets of its pairs' source blocks in the right-hand-side
+  // buffer: x = pair 0 (low / high 16 bits: kb 512 | (kb & 7) << 5, the kernel's bank swizzle),
+  // y = pair 1 (one-product slots); absent blocks point at block 0 with zero values.
+  int hs_na[4] = {0, 0, 0, 0}, hs_nb[4] = {0, 0, 0, 0};
+  int hs_slots = 0;                  // slots per warp = sum_j hs_na[j] + hs_nb[j]
+  std::vector<uint8_t> hs_rows;      // [4][32] output block row of (row slot, warp), 255 = none
+  std::vector<uint32_t> hs_desc;     // [warps][32 lanes][4]: descriptors of slots lane (words 0, 1) and lane + 32 (words 2, 3)
+  std::vector<uint32_t> hs_val;      // [warps][hs_slots][32 lanes][4]
+  std::vector<int32_t> hp_ptr;       // [nvb][4] pair ranges for npfem_plan_query: three-product [0],[1]), one-product [2],[3])
+  std::vector<uint32_t> hp_col_a;    // [pairs A] source blocks kb1 | kb2 << 16 (0xffff = none)
+  std::vector<uint32_t> hp_val_a;    // [pairs A][32 lanes][4]: B fragment hi (2 words), lo (2 words)
+  std::vector<uint32_t> hp_col_b;    // [pairs B]
+  std::vector<uint32_t> hp_val_b;    // [pairs B][32 lanes][2]: B fragment hi
+  std::vector<float> hp_scale;       // [n] 2^-k of the row's scaling 2^k (internal numbering)
+  int n_op_blocks_h1 = 0;            // kept blocks applied as one fp16 product
   int n_op_blocks = 0;               // kept blocks (without the zero padding blocks)
   int n_op_blocks_x1 = 0;            // of those, blocks applied as one TF32 product
   int op_nnz = 0;
@@ -94,7 +122,8 @@ int build_plan(int n_verts, int n_tris, const int32_t* tris, const double* rest_
 //                         A-fragment order ([nvb][32] float4)
 //   rb   max(E*64, NP*64) element results of the EVEN cells during the local step, then the
 //                         tf32 low parts of the right-hand sides, then the increments of d
-//   red  [5][32] float4   per-warp partial sums of the volume reductions, then [5] float4 centroids
+//   red  [5][32] float4   per-warp partial sums of the volume reductions, then [5] float4 centroids,
+//                         then [5] uint32: bits of max |r| per cell (global_mode 3: fp16 scaling)
 // The inertial prediction s and the correction d are private to the thread that owns the vertex
 // and live in tensor memory (TMEM), 32 columns per group of 4 warps.
 constexpr int kElemGroups = 9;
@@ -111,7 +140,7 @@ inline SmemLayout smem_layout(int n, int E, int nvb, int k) {
   const int rbuf = E * 64 > NP * 64 ? E * 64 : NP * 64;   // both buffers hold [4][E] element results
   L.ra = off; off += rbuf;
   L.rb = off; off += rbuf;
-  L.red = off; off += kMaxCellsPerCta * 32 * 16 + kMaxCellsPerCta * 16;   // + the cells' centroids
+  L.red = off; off += kMaxCellsPerCta * 32 * 16 + kMaxCellsPerCta * 16 + 32;   // + the cells' centroids + residual maxima (global_mode 3)
   L.total = off;
   return L;
 }

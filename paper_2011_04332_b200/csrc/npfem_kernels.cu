@@ -23,6 +23,9 @@
 // accumulate).  s, d, the elastic residual and u0, private to the owner thread, live in tensor
 // memory (TMEM).
 #include <cstdint>
+#include <cstring>
+
+#include <cuda_fp16.h>
 
 #include "npfem_device.cuh"
 
@@ -39,6 +42,29 @@ __device__ __forceinline__ void jitter_sleep(int seed, int phase, int warp) {
   hsh ^= hsh >> 13; hsh *= 0x5bd1e995u; hsh ^= hsh >> 15;
   __nanosleep(hsh & 2047u);
 }
+// Diagnostic build (-DNPFEM_PHASE_CLOCKS, never the shipped library): thread 0 of every CTA adds the
+// clock64() ticks between marks to g_phase[] (one slot per phase of an iteration), read back with
+// npfem_debug_phase_clocks (profiles/ quotes these as "phase clocks").
+#ifdef NPFEM_PHASE_CLOCKS
+__device__ unsigned long long g_phase[16];
+#define NPFEM_PHASE(i)                                                          \
+  do {                                                                          \
+    if (tid == 0) {                                                             \
+      const long long t_now = clock64();                                        \
+      atomicAdd(&g_phase[i], (unsigned long long)(t_now - t_phase));            \
+      t_phase = t_now;                                                          \
+    }                                                                           \
+  } while (0)
+#define NPFEM_PDBG(bit) (P.dbg & (bit))
+#else
+#define NPFEM_PHASE(i) do { } while (0)
+#define NPFEM_PDBG(bit) 0
+#endif
+#ifndef NPFEM_OP_DEPTH
+#define NPFEM_OP_DEPTH 4
+#endif
+constexpr int kOpDepth = NPFEM_OP_DEPTH;   // slots of the operator stream a warp loads per batch (MODE 3)
+
 #define NPFEM_SYNC()                                                    \
   do {                                                                  \
     __syncthreads();                                                    \
@@ -63,10 +89,15 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   unsigned char* const rbb = smem_raw + P.L.rb;                        // element results (even cells) / rhs lo / delta d
   float* const rb = reinterpret_cast<float*>(rbb);
   float4* const red = reinterpret_cast<float4*>(smem_raw + P.L.red);   // [5][32] partial sums
+  // MODE 3: bits of max |r| per cell (the right-hand sides are scaled into the fp16 range per cell)
+  uint32_t* const smax = reinterpret_cast<uint32_t*>(smem_raw + P.L.red + kMaxCellsPerCta * 33 * 16);
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
   int jphase = 0;   // barrier counter of the schedule-jitter debug option
+#ifdef NPFEM_PHASE_CLOCKS
+  long long t_phase = clock64();
+#endif
   const int n = P.n, E = P.E, nvb = P.nvb, NP = nvb * 8;
   const int cell0 = blockIdx.x * P.k;
   const int kact = min(P.k, P.n_cells - cell0);
@@ -95,8 +126,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   for (int i = tid; i < kElemGroups * E; i += blockDim.x)
     reinterpret_cast<float4*>(smem_raw + P.L.ec)[i] = P.elem_c[i];
   for (int i = tid; i < NP * 16; i += blockDim.x) ra[i] = 0.0f;
-  for (int i = tid; i < P.k * NP; i += blockDim.x)
-    reinterpret_cast<float4*>(z4b)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (tid < 8) smax[tid] = 0u;
 
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   NPFEM_SYNC();
@@ -210,6 +240,8 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
   const float vol_dtol2 = (float)n * vol_dlen * vol_dlen;
   const bool use_vol = P.w_volume > 0.0f;
   const float4* const ec_t = ecs + (is_e ? tid : 0);
+  const float nmh2 = -__uint_as_float(P.vrole[2 * v + 1].w);   // -(m/h^2) (with damping: -m (1/h^2 + c_alpha/h))
+  NPFEM_PHASE(0);   // prologue
   for (int it = 0; it < P.n_iters; ++it) {
     // local step.  Pipeline over the CTA's cells, one barrier per cell:
     //   [elements(0) -> out B; volume gradient(0), partial sums] |
@@ -222,6 +254,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     // counts, [1] = ring offsets 0..5 (3 words) + m/h^2.
     F3 g = {0.f, 0.f, 0.f}, zv = {0.f, 0.f, 0.f};
     uint4 vr0;
+    if (MODE == 3 && tid < kMaxCellsPerCta) smax[tid] = 0u;   // read last by the owner update, before its barrier
     // element results alternate between two buffers (rb, and ra, which is idle until the split),
     // so the vertex phase of cell c and the element pass of cell c+1 share one barrier interval
     auto elements_and_gradient = [&](int cc) {
@@ -243,6 +276,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     };
     elements_and_gradient(0);
     NPFEM_SYNC();
+    NPFEM_PHASE(1);   // element pass + volume gradient of the first cell
     for (int c = 0; c < kact; ++c) {
       const unsigned char* zc = z4b + c * cellz;
       const unsigned char* outb = (c & 1) ? rab : rbb;
@@ -325,33 +359,68 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
           if (t > 0.f) ev = fma3(P.w_coll * t, nn, ev);
         }
       }
-      // elastic residual of the cell's vertices, e = sum of element results + w_vol D, parked in
-      // the owner's TMEM columns 32 + 3c .. (the fourth column written belongs to the next cell,
-      // which overwrites it later in this same pass)
-      tmem_st4(ta + 32 + 3 * c, fmaf(P.w_volume, D.x, ev.x), fmaf(P.w_volume, D.y, ev.y),
-               fmaf(P.w_volume, D.z, ev.z), 0.0f);
+      // right-hand side of the global step for the cell's vertices, r = e - (m/h^2) d with the
+      // elastic residual e = sum of element results + w_vol D, parked in the owner's TMEM columns
+      // 32 + 3c .. (the fourth column written belongs to the next cell, which overwrites it later
+      // in this same pass)
+      {
+        float d0, d1, d2, d3;
+        tmem_ld4(ta + 16 + 3 * c, d0, d1, d2, d3);
+        float rx = fmaf(nmh2, d0, fmaf(P.w_volume, D.x, ev.x));
+        float ry = fmaf(nmh2, d1, fmaf(P.w_volume, D.y, ev.y));
+        float rz = fmaf(nmh2, d2, fmaf(P.w_volume, D.z, ev.z));
+        if (DAMP) {
+          tmem_ld4(ta + 64 + 3 * c, d0, d1, d2, d3);
+          rx += d0; ry += d1; rz += d2;
+        }
+        tmem_st4(ta + 32 + 3 * c, rx, ry, rz, 0.0f);
+        if (MODE == 3) {   // max |r| of the cell: the fp16 split below scales by a power of two
+          uint32_t mb = __float_as_uint(fmaxf(fmaxf(fabsf(rx), fabsf(ry)), fabsf(rz)));
+          mb = __reduce_max_sync(0xffffffffu, mb);
+          if (lane == 0) atomicMax(&smax[c], mb);
+        }
+      }
       if (c + 1 < kact) elements_and_gradient(c + 1);
       NPFEM_SYNC();   // out(c) consumed; out(c+1) and the partial sums of cell c+1 complete
     }
 
-    // right-hand sides of the global step, r = e - (m/h^2) d, split into tf32 high and low parts and
-    // written in mma A-fragment order (hi -> ra, lo -> rb; both element buffers are dead now).
-    // Round-to-nearest on the 13 dropped mantissa bits; lo = x - hi is exact.
+    NPFEM_PHASE(2);   // vertex phase(c) + element pass(c+1), one barrier per cell
+    // right-hand sides of the global step: r, split into a high and a low part and written in mma
+    // A-fragment order (both element buffers are dead now).
+    // MODE 1/2: tf32 hi -> ra, lo -> rb; round-to-nearest on the 13 dropped mantissa bits, lo = x - hi
+    // is exact.  MODE 3: scaled by the cell's 2^k so that max |r| lands in [2^13, 2^14), then
+    // hi = fp16(x), lo = fp16(x - hi) (x to 2^-24 relative), both into ra: source block kb holds a hi
+    // plane and, 256 bytes further, a lo plane of 32 chunks of 8 bytes {col g, col g+8}, each word
+    // the vertices 2t, 2t+1 of the block; chunk index (4 g + t) ^ 4 (kb & 7): the xor keeps the
+    // 16-bit stores of a warp (4 source blocks x 4 t) on distinct banks.
     {
-      float ee[16], dd[16];
-      tmem_ld16(ta + 32, ee);
-      if (DAMP) {
-        tmem_ld16(ta + 64, dd);
+      float rr[16];
+      tmem_ld16(ta + 32, rr);
+      if (MODE == 3) {
+        if (isvp && !NPFEM_PDBG(32)) {
+          float sc[kMaxCellsPerCta];
 #pragma unroll
-        for (int m = 0; m < 15; ++m) ee[m] += dd[m];
-      }
-      tmem_ld16(ta + 16, dd);
-      const float nmh2 = -__uint_as_float(P.vrole[2 * v + 1].w);
-      if (isvp) {
+          for (int c = 0; c < kMaxCellsPerCta; ++c) {
+            const uint32_t ec_ = min(max(smax[c] >> 23, 14u), 254u);
+            sc[c] = __uint_as_float((267u - ec_) << 23);
+          }
+          const uint32_t sw = ((uint32_t)(v >> 3) & 7u) * 32u;
+          unsigned char* const wb = rab + (v >> 3) * 512 + ((v & 7) >> 1) * 8 + (v & 1) * 2;
+#pragma unroll
+          for (int m = 0; m < kRhs; ++m) {
+            const float x = m < 15 ? rr[m] * sc[m / 3] : 0.0f;
+            const __half hi = __float2half_rn(x);
+            const __half lo = __float2half_rn(x - __half2float(hi));
+            unsigned char* const w = wb + (((uint32_t)(m & 7) * 32u) ^ sw) + (m >> 3) * 4;
+            *reinterpret_cast<__half*>(w) = hi;
+            *reinterpret_cast<__half*>(w + 256) = lo;
+          }
+        }
+      } else if (isvp) {
 #pragma unroll
         for (int m = 0; m < kRhs; ++m) {
           const int idx = fbase + (m & 7) * 16 + (m >> 3);
-          const float x = m < 15 ? fmaf(nmh2, dd[m], ee[m]) : 0.0f;
+          const float x = m < 15 ? rr[m] : 0.0f;
           const float hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
           ra[idx] = hi;
           rb[idx] = x - hi;
@@ -360,10 +429,76 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     }
     NPFEM_SYNC();
 
+    NPFEM_PHASE(3);   // split + barrier
     // global step: delta d = T r with T = A_sys^-1 in 8x8 blocks.  One warp per block row of 8
     // output vertices (up to 4 rows per warp): mma m16n8k8, M = the 16 right-hand-side columns,
     // N = 8 output vertices, K = 8 source vertices per operator block (block_run above).
-    const int g8 = lane >> 2, t4 = lane & 3;
+    int tid_p = tid;
+    asm volatile("" : "+r"(tid_p));   // everything the product derives from the thread index is formed here, per
+                                      // iteration, instead of being hoisted and kept live across the element pass
+    const int lane_p = tid_p & 31, warp_p = tid_p >> 5;
+    const int g8 = lane_p >> 2, t4 = lane_p & 3;
+    if constexpr (MODE == 3) {
+      // the warp's operator stream: slots of 512 bytes of B fragments, consumed in order.  The
+      // stream has the same shape for every warp (per row slot
+      // j: hs_na[j] three-product slots, then hs_nb[j] one-product slots), so every branch below
+      // is uniform; the slot descriptors (<= 64 slots per warp) sit in four registers, lane l
+      // holding those of slots l and l + 32, and are broadcast by shuffle; a finished block row
+      // goes straight to the owners' hand-off buffer (rb is not read in this phase)
+      const int Q = NPFEM_PDBG(16) ? 0 : P.hs_slots;
+      const uint4* const vp = P.hs_val + (size_t)warp_p * Q * 32 + lane_p;
+      // (x, y) slot lane, (z, w) slot lane + 32.  The identity shuffles re-home the four words from
+      // the load's scoreboard to registers no pending load guards: ptxas otherwise makes every
+      // later read of them wait for the newest stream loads as well (measured: the whole L2
+      // latency per slot).
+      uint4 dreg = __ldg(P.hs_desc + warp_p * 32 + lane_p);
+      dreg.x = __shfl_sync(0xffffffffu, dreg.x, lane_p); dreg.y = __shfl_sync(0xffffffffu, dreg.y, lane_p);
+      dreg.z = __shfl_sync(0xffffffffu, dreg.z, lane_p); dreg.w = __shfl_sync(0xffffffffu, dreg.w, lane_p);
+      const uint32_t lane8 = (uint32_t)lane_p * 8u;
+      // Batches of kOpDepth slots: all loads of a batch are issued back to back, then the batch is
+      // consumed.  No load is in flight while a warp computes -- deliberately: ptxas guards every
+      // register a load wrote with a scoreboard that later loads re-use, so that in a software-
+      // pipelined ring the consumer of the OLDEST load also waits for the newest (measured: one
+      // whole L2 latency per slot, whatever the depth).  The latency of a batch is covered by the
+      // other warps of the sub-partition, which sit in other batches.  (Measured in isolation: the
+      // loop is bound by the SM's load/store data path, which the 512-byte stream loads (5.8 cycles
+      // each) and the 256-byte right-hand-side loads (2 cycles each) share; starting the warps of a
+      // sub-partition staggered changed nothing.)
+      {
+        float acc[4] = {0.f, 0.f, 0.f, 0.f}, accx[4] = {0.f, 0.f, 0.f, 0.f};
+        int j = 0, qa_end = P.hs_na[0], q_end = P.hs_na[0] + P.hs_nb[0];
+        for (int q = 0; q < Q; q += kOpDepth) {
+          uint4 rv[kOpDepth];
+#pragma unroll
+          for (int u = 0; u < kOpDepth; ++u)
+            if (q + u < Q) rv[u] = ldg_stream(vp + (q + u) * 32);
+#pragma unroll
+          for (int u = 0; u < kOpDepth; ++u) {
+            if (q + u < Q) {
+              uint2 d;
+              d.x = __shfl_sync(0xffffffffu, q + u < 32 ? dreg.x : dreg.z, (q + u) & 31);
+              d.y = q + u < qa_end ? 0u : __shfl_sync(0xffffffffu, q + u < 32 ? dreg.y : dreg.w, (q + u) & 31);
+              if (q + u < qa_end) slot_mma3(acc, accx, rv[u], d.x, rab, lane8, NPFEM_PDBG(0xff));
+              else slot_mma1(acc, accx, rv[u], d, rab, lane8, NPFEM_PDBG(0xff));
+              if (q + u + 1 == q_end) {
+                const int ib = P.hs_rows[j * 32 + warp_p];
+                if (ib != 255) {
+                  const int i0 = ib * 8 + 2 * t4;
+                  *reinterpret_cast<float2*>(rb + g8 * NP + i0) = make_float2(acc[0] + accx[0], acc[1] + accx[1]);
+                  if (g8 < 7)
+                    *reinterpret_cast<float2*>(rb + (g8 + 8) * NP + i0) = make_float2(acc[2] + accx[2], acc[3] + accx[3]);
+                }
+#pragma unroll
+                for (int x = 0; x < 4; ++x) { acc[x] = 0.f; accx[x] = 0.f; }
+                ++j;
+                if (j < 4) { qa_end = q_end + P.hs_na[j]; q_end = qa_end + P.hs_nb[j]; }
+              }
+            }
+          }
+        }
+      }
+      NPFEM_PHASE(4);   // operator product, warp 0's own rows
+    } else {
     float acc[4][4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -401,6 +536,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         }
       }
     }
+    NPFEM_PHASE(4);   // operator product, warp 0's own rows
     NPFEM_SYNC();   // every warp is done reading the right-hand sides
 
     // hand the increments to the vertex owners: dd[m][NP] over the dead lo buffer
@@ -413,15 +549,28 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         if (g8 < 7) *reinterpret_cast<float2*>(rb + (g8 + 8) * NP + i0) = make_float2(acc[j][2], acc[j][3]);
       }
     }
+    }
     NPFEM_SYNC();
-
+    NPFEM_PHASE(5);   // hand-off + wait for the slowest warp of the product
     // owner update: d += delta d, z = s + d
     {
       float sv[16], dv[16];
       tmem_ld16(ta, sv);
       tmem_ld16(ta + 16, dv);
+      if (MODE == 3) {   // undo the scaling of the operator row (2^-k_v) and of the cell's right-hand sides
+        const float hs = NPFEM_PDBG(0xff) ? 0.0f : P.hp_scale[v];   // ablation runs leave d alone
+        float fac[kMaxCellsPerCta];
 #pragma unroll
-      for (int m = 0; m < 15; ++m) dv[m] += rb[m * NP + v];
+        for (int c = 0; c < kMaxCellsPerCta; ++c) {
+          const uint32_t ec_ = min(max(smax[c] >> 23, 14u), 254u);
+          fac[c] = hs * __uint_as_float((ec_ - 13u) << 23);
+        }
+#pragma unroll
+        for (int m = 0; m < 15; ++m) dv[m] = fmaf(rb[m * NP + v], fac[m / 3], dv[m]);
+      } else {
+#pragma unroll
+        for (int m = 0; m < 15; ++m) dv[m] += rb[m * NP + v];
+      }
       if (isvp) {
 #pragma unroll
         for (int c = 0; c < kMaxCellsPerCta; ++c)
@@ -432,6 +581,7 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
       tmem_st16(ta + 16, dv);
     }
     NPFEM_SYNC();
+    NPFEM_PHASE(6);   // owner update
   }
 
   // ---- epilogue: x_n+1 = x_n + (u0 + d), v_n+1 = (u0 + d)/h, staged in caller order through
@@ -499,6 +649,28 @@ cudaError_t launch_vertex_areas(const DevParams& p, int threads, float* areas, c
   return cudaGetLastError();
 }
 
+#ifdef NPFEM_PHASE_CLOCKS
+static int g_dbg_host = 0;
+#endif
+cudaError_t read_phase_clocks(unsigned long long* out16, int reset) {
+#ifdef NPFEM_PHASE_CLOCKS
+  if (reset >= 0x100) {   // diagnostic: set the ablation mask of the operator product (low byte)
+    g_dbg_host = reset & 0xff;
+    return cudaSuccess;
+  }
+  cudaError_t e = cudaMemcpyFromSymbol(out16, g_phase, sizeof(unsigned long long) * 16);
+  if (e != cudaSuccess) return e;
+  if (reset) {
+    unsigned long long zero[16] = {};
+    e = cudaMemcpyToSymbol(g_phase, zero, sizeof(zero));
+  }
+  return e;
+#else
+  (void)out16; (void)reset;
+  return cudaErrorNotSupported;
+#endif
+}
+
 cudaError_t configure_kernels(int smem_bytes) {
   cudaError_t e;
   (void)smem_bytes;
@@ -510,13 +682,21 @@ cudaError_t configure_kernels(int smem_bytes) {
   NPFEM_CFG(1, 672, 0) NPFEM_CFG(1, 1024, 0) NPFEM_CFG(2, 672, 0) NPFEM_CFG(2, 1024, 0)
   NPFEM_CFG(1, 672, 1) NPFEM_CFG(1, 1024, 1) NPFEM_CFG(2, 672, 1) NPFEM_CFG(2, 1024, 1)
   NPFEM_CFG(1, 672, 2) NPFEM_CFG(1, 1024, 2) NPFEM_CFG(2, 672, 2) NPFEM_CFG(2, 1024, 2)
+  NPFEM_CFG(3, 672, 0) NPFEM_CFG(3, 1024, 0) NPFEM_CFG(3, 672, 1) NPFEM_CFG(3, 1024, 1)
+  NPFEM_CFG(3, 672, 2) NPFEM_CFG(3, 1024, 2)
 #undef NPFEM_CFG
   return cudaSuccess;
 }
 
-cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mode,
+cudaError_t launch_step(const DevParams& p_in, int threads, int smem_bytes, int mode,
                         cudaStream_t stream) {
-  if (p.n_cells <= 0) return cudaSuccess;
+  if (p_in.n_cells <= 0) return cudaSuccess;
+#ifdef NPFEM_PHASE_CLOCKS
+  DevParams p = p_in;
+  p.dbg = g_dbg_host;
+#else
+  const DevParams& p = p_in;
+#endif
   const int grid = (p.n_cells + p.k - 1) / p.k;
   const int feat = p.damped ? 1 : (p.coll_n != nullptr || p.jitter != 0 || p.hard != 0.0f) ? 2 : 0;
 #define NPFEM_LAUNCH(MODE, MAXT)                                                                  \
@@ -526,9 +706,9 @@ cudaError_t launch_step(const DevParams& p, int threads, int smem_bytes, int mod
     else npfem_step_kernel<MODE, MAXT, 0><<<grid, threads, smem_bytes, stream>>>(p);              \
   } while (0)
   if (threads <= 672) {
-    if (mode == 2) NPFEM_LAUNCH(2, 672); else NPFEM_LAUNCH(1, 672);
+    if (mode == 3) NPFEM_LAUNCH(3, 672); else if (mode == 2) NPFEM_LAUNCH(2, 672); else NPFEM_LAUNCH(1, 672);
   } else {
-    if (mode == 2) NPFEM_LAUNCH(2, 1024); else NPFEM_LAUNCH(1, 1024);
+    if (mode == 3) NPFEM_LAUNCH(3, 1024); else if (mode == 2) NPFEM_LAUNCH(2, 1024); else NPFEM_LAUNCH(1, 1024);
   }
 #undef NPFEM_LAUNCH
   return cudaGetLastError();

@@ -22,6 +22,7 @@ struct DevParams {
   float cbh;                               // c_beta / h (stiffness-proportional damping, A-20)
   int damped;                              // c_alpha != 0 or c_beta != 0
   int jitter;                              // debug: seed of the per-warp sleeps after every barrier (0 = off)
+  int dbg;                                 // diagnostic builds: ablation mask of the MODE 3 product (0 in the shipped library)
   const uint16_t* perm;                    // [NP] internal -> caller vertex (padding: 0)
   const float4* elem_c;                    // [kElemGroups][E] element constants (npfem_api.cu)
   const float* h2_over_m;                  // [NP]
@@ -35,6 +36,13 @@ struct DevParams {
   const int* blk_ptr;                      // [nvb][3]: first 3xTF32 block, first 1xTF32 block, end
   const uint16_t* blk_col;                 // [n_blocks_padded]
   const float* blk_val;                    // [n_blocks_padded][64]
+  // global_mode 3: per-warp operator streams of uniform shape (npfem_internal.h)
+  const uint4* hs_val;                     // [warps][hs_slots][32]: B fragments, 16 bytes per lane and slot
+  const uint4* hs_desc;                    // [warps][32 lanes]: descriptors of slots lane (x, y) and lane + 32 (z, w)
+  int hs_slots;                            // slots per warp (<= 64)
+  int hs_na[4], hs_nb[4];                  // per row slot: three-product slots, one-product slots
+  uint8_t hs_rows[4 * 32];                 // [row slot][warp] -> output block row, 255 = none
+  const float* hp_scale;                   // [NP] 2^-k of the operator row's scaling
   float* pos;
   float* vel;
   const float* fext;
@@ -44,6 +52,10 @@ struct DevParams {
   float hard;                              // strain hardening beta (A-23)
   SmemLayout L;
 };
+
+// Diagnostic builds only (-DNPFEM_PHASE_CLOCKS): accumulated clock64() ticks per phase of the step
+// kernel, summed over CTAs and iterations; cudaErrorNotSupported in the shipped library.
+cudaError_t read_phase_clocks(unsigned long long* out16, int reset);
 
 // Opt the kernels into their dynamic shared memory once per process.  Returns a cudaError_t.
 cudaError_t configure_kernels(int smem_bytes);

@@ -45,6 +45,29 @@ inline double cot_corner(V3 p, V3 q, V3 r) {
 // multiple of 8 when the subset is large enough), recursively.  Consecutive groups of 8/16/32
 // internal indices are then compact surface patches, which is what keeps the 8x8 blocks of the
 // numerically sparse A_sys^-1 few.
+// fp32 -> fp16 bits, round to nearest even (subnormals included); |f| < 65520 by construction.
+uint16_t half_bits(float f) {
+  uint32_t x;
+  std::memcpy(&x, &f, 4);
+  const uint16_t sign = (uint16_t)((x >> 16) & 0x8000u);
+  x &= 0x7fffffffu;
+  if (x >= 0x477ff000u) return (uint16_t)(sign | 0x7c00u);   // rounds to >= 65536: infinity
+  if (x < 0x38800000u) {                                      // below 2^-14: fp16 subnormal, unit 2^-24
+    float a;
+    std::memcpy(&a, &x, 4);
+    return (uint16_t)(sign | (uint32_t)std::nearbyint(a * 16777216.0f));
+  }
+  uint32_t hb = (((x >> 23) - 112u) << 10) | ((x & 0x7fffffu) >> 13);
+  const uint32_t rem = x & 0x1fffu;
+  if (rem > 0x1000u || (rem == 0x1000u && (hb & 1u))) ++hb;   // a carry into the exponent is the right result
+  return (uint16_t)(sign | hb);
+}
+float half_value(uint16_t hb) {
+  const int e = (hb >> 10) & 0x1f, m = hb & 0x3ff;
+  const float v = e == 0 ? std::ldexp((float)m, -24) : std::ldexp((float)(m | 0x400), e - 25);
+  return (hb & 0x8000u) ? -v : v;
+}
+
 struct Bisector {
   const std::vector<std::vector<int>>& adj;
   std::vector<int> mark, dist;
@@ -146,7 +169,7 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
   if (o.volume_inner_iters > 32) o.volume_inner_iters = 32;
   if (o.cells_per_cta < 0 || o.cells_per_cta > kMaxCellsPerCta)
     return fail(NPFEM_EINVAL, "cells_per_cta must be 0..5");
-  if (o.global_mode < 0 || o.global_mode > 2) return fail(NPFEM_EINVAL, "global_mode must be 0..2");
+  if (o.global_mode < 0 || o.global_mode > 3) return fail(NPFEM_EINVAL, "global_mode must be 0..3");
   if (o.pair_triangles < 0 || o.pair_triangles > 2) return fail(NPFEM_EINVAL, "pair_triangles must be 0..2");
   P->tris_ext.assign(tris, tris + 3 * T);
   auto Xv = [&](int v) { return V3{X[3 * v], X[3 * v + 1], X[3 * v + 2]}; };
@@ -439,6 +462,108 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     }
   }
 
+  // ---- the same operator for global_mode 3: two-term fp16 split on mma m16n8k16 (K = 16 = a PAIR
+  //      of source blocks per instruction).  x = hi + lo with hi = fp16(x), lo = fp16(x - hi)
+  //      represents x to 2^-24 relative, so hi*hi + hi*lo + lo*hi with fp32 accumulation is
+  //      fp32-equivalent (the dropped lo*lo is 2^-24 of the product).  A product of the hi parts
+  //      alone errs by <= 2^-11 relative (each operand rounded to 11 bits), so blocks are moved to
+  //      the one-product run, smallest first, while their l1 mass stays <= 2^-13 of the l1 norm of
+  //      every row of the block row: total error <= 2^-24 ||row||_1 |r|_max, one fp32 rounding.
+  //      Row i is scaled by 2^k_i so that its largest entry lies in [2^13, 2^14) (fp16 normal range
+  //      reaches down to 2^-14: 27 binades below, more than the 24 the drop rule leaves); the
+  //      kernel scales the right-hand sides likewise per cell and undoes both with hp_scale.
+  //      A run with an odd number of blocks ends with a half-empty pair.
+  {
+    const double tier_tol = std::ldexp(1.0, -13);
+    auto Tint = [&](int i, int j) {
+      return (i < n && j < n) ? Tinv[(size_t)P->perm[i] * n + P->perm[j]] : 0.0;
+    };
+    std::vector<int> kexp(nvb * 8, 0);
+    P->hp_scale.assign(n, 1.0f);
+    for (int i = 0; i < n; ++i) {
+      double mx = 0.0;
+      for (int j = 0; j < n; ++j) mx = std::max(mx, std::fabs(Tint(i, j)));
+      int e = 0;
+      if (mx > 0.0) std::frexp(mx, &e);   // mx = f 2^e, f in [0.5, 1)
+      kexp[i] = 14 - e;                   // mx 2^k in [2^13, 2^14)
+      P->hp_scale[i] = (float)std::ldexp(1.0, -kexp[i]);
+    }
+    P->hp_ptr.assign(4 * (size_t)nvb, 0);
+    P->hp_col_a.clear(); P->hp_val_a.clear(); P->hp_col_b.clear(); P->hp_val_b.clear();
+    P->n_op_blocks_h1 = 0;
+    // B fragment of mma.m16n8k16 (col): lane = 4 g + t holds b0 = (k = 2t, 2t+1; n = g) from the first
+    // source block and b1 = (k = 2t+8, 2t+9; n = g) from the second; low half = lower k.
+    auto emit_pair = [&](int ib, int jb1, int jb2, bool full) {
+      std::vector<uint32_t>& val = full ? P->hp_val_a : P->hp_val_b;
+      (full ? P->hp_col_a : P->hp_col_b)
+          .push_back((uint32_t)(jb1 < 0 ? 0xffff : jb1) | ((uint32_t)(jb2 < 0 ? 0xffff : jb2)) << 16);
+      const int words = full ? 4 : 2;
+      size_t base = val.size();
+      val.resize(base + 32 * (size_t)words, 0u);
+      for (int l = 0; l < 32; ++l) {
+        const int g = l >> 2, t = l & 3, i = ib * 8 + g;
+        for (int half = 0; half < 2; ++half) {
+          const int jb = half ? jb2 : jb1;
+          if (jb < 0) continue;
+          uint32_t hi = 0, lo = 0;
+          for (int q = 0; q < 2; ++q) {
+            const float x = (float)std::ldexp(Tint(i, jb * 8 + 2 * t + q), i < n ? kexp[i] : 0);
+            const uint16_t hb = half_bits(x);
+            const uint16_t lb = half_bits(x - half_value(hb));
+            hi |= (uint32_t)hb << (16 * q);
+            lo |= (uint32_t)lb << (16 * q);
+          }
+          val[base + (size_t)l * words + half] = hi;
+          if (full) val[base + (size_t)l * words + 2 + half] = lo;
+        }
+      }
+    };
+    for (int ib = 0; ib < nvb; ++ib) {
+      std::vector<int> cols;
+      for (int jb = 0; jb < nvb; ++jb)
+        if (bmask[(size_t)ib * nvb + jb]) cols.push_back(jb);
+      std::vector<std::array<double, 8>> mass(cols.size());
+      std::array<double, 8> rowl1{};
+      for (size_t q = 0; q < cols.size(); ++q)
+        for (int r = 0; r < 8; ++r) {
+          double m = 0.0;
+          for (int cc = 0; cc < 8; ++cc) m += std::fabs(Tint(ib * 8 + r, cols[q] * 8 + cc));
+          mass[q][r] = m;
+          rowl1[r] += m;
+        }
+      std::vector<int> order(cols.size());
+      std::iota(order.begin(), order.end(), 0);
+      auto bmax = [&](int q) { return *std::max_element(mass[q].begin(), mass[q].end()); };
+      std::sort(order.begin(), order.end(), [&](int p, int q) {
+        double mp = bmax(p), mq = bmax(q);
+        return mp != mq ? mp < mq : p < q;
+      });
+      std::vector<uint8_t> single(cols.size(), 0);
+      std::array<double, 8> cum{};
+      for (int q : order) {
+        bool ok = cols[q] != ib;   // the diagonal block always takes three products
+        for (int r = 0; r < 8 && ok; ++r)
+          if (rowl1[r] > 0.0 && cum[r] + mass[q][r] > tier_tol * rowl1[r]) ok = false;
+        if (!ok) break;
+        for (int r = 0; r < 8; ++r) cum[r] += mass[q][r];
+        single[q] = 1;
+      }
+      for (int pass = 0; pass < 2; ++pass) {
+        std::vector<uint32_t>& colv = pass ? P->hp_col_b : P->hp_col_a;
+        P->hp_ptr[4 * (size_t)ib + 2 * pass] = (int32_t)colv.size();
+        std::vector<int> run;
+        for (size_t q = 0; q < cols.size(); ++q)
+          if ((int)single[q] == pass) run.push_back(cols[q]);
+        P->n_op_blocks_h1 += pass ? (int)run.size() : 0;
+        int run_pairs = 0;
+        for (size_t q = 0; q < run.size(); q += 2, ++run_pairs)
+          emit_pair(ib, run[q], q + 1 < run.size() ? run[q + 1] : -1, pass == 0);
+        (void)run_pairs;
+        P->hp_ptr[4 * (size_t)ib + 2 * pass + 1] = (int32_t)colv.size();
+      }
+    }
+  }
+
   // ---- per-vertex constants (internal numbering)
   P->h2_over_m.resize(n);
   P->m_over_h2.resize(n);
@@ -689,7 +814,69 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     return fail(NPFEM_ELIMIT, "cell state does not fit the shared memory of one SM");
   P->cells_per_cta = k;
   P->smem_bytes = smem_layout(n, E, nvb, k).total;
-  P->global_mode = o.global_mode ? o.global_mode : 2;
+
+  // ---- global_mode 3: per-warp operator streams of uniform shape (npfem_internal.h)
+  {
+    const int W = P->threads / 32;
+    const int J = (nvb + W - 1) / W;
+    if (J > 4 || W > 32) return fail(NPFEM_ELIMIT, "internal: more than 4 operator block rows per warp");
+    auto pairs_a = [&](int ib) { return P->hp_ptr[4 * (size_t)ib + 1] - P->hp_ptr[4 * (size_t)ib]; };
+    auto pairs_b = [&](int ib) { return P->hp_ptr[4 * (size_t)ib + 3] - P->hp_ptr[4 * (size_t)ib + 2]; };
+    std::vector<int> order(nvb);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int p, int q) {   // by mma count, longest first
+      return 3 * pairs_a(p) + pairs_b(p) > 3 * pairs_a(q) + pairs_b(q);
+    });
+    P->hs_rows.assign(4 * 32, 255);
+    for (int j = 0; j < 4; ++j) { P->hs_na[j] = 0; P->hs_nb[j] = 0; }
+    for (int r = 0; r < nvb; ++r) {
+      const int j = r / W, w = r % W, ib = order[r];
+      P->hs_rows[(size_t)j * 32 + w] = (uint8_t)ib;
+      P->hs_na[j] = std::max(P->hs_na[j], pairs_a(ib));
+      P->hs_nb[j] = std::max(P->hs_nb[j], (pairs_b(ib) + 1) / 2);
+    }
+    P->hs_slots = 0;
+    for (int j = 0; j < 4; ++j) P->hs_slots += P->hs_na[j] + P->hs_nb[j];
+    const int Q = P->hs_slots;
+    P->hs_desc.assign((size_t)W * 128, 0u);
+    auto dword = [&](int w, int q, int x) -> uint32_t& {   // descriptor word x of slot q of warp w
+      return P->hs_desc[((size_t)w * 32 + (q & 31)) * 4 + 2 * ((q >> 5) & 1) + x];
+    };
+    P->hs_val.assign((size_t)W * Q * 128, 0u);
+    auto colword = [](uint32_t kb) { return kb == 0xffffu ? 0u : (kb << 9 | (kb & 7u) << 5); };
+    for (int w = 0; w < W; ++w) {
+      int q0 = 0;
+      for (int j = 0; j < 4; ++j) {
+        const int ib = P->hs_rows[(size_t)j * 32 + w];
+        if (ib != 255) {
+          const int a0 = P->hp_ptr[4 * (size_t)ib], b0 = P->hp_ptr[4 * (size_t)ib + 2];
+          for (int u = 0; u < pairs_a(ib); ++u) {
+            const size_t slot = (size_t)w * Q + q0 + u;
+            const uint32_t c = P->hp_col_a[a0 + u];
+            if (q0 + u < kMaxOpSlots) dword(w, q0 + u, 0) = colword(c & 0xffffu) | colword(c >> 16) << 16;
+            for (int l = 0; l < 32; ++l)
+              for (int x = 0; x < 4; ++x)
+                P->hs_val[(slot * 32 + l) * 4 + x] = P->hp_val_a[((size_t)(a0 + u) * 32 + l) * 4 + x];
+          }
+          for (int u = 0; u < pairs_b(ib); ++u) {
+            const size_t slot = (size_t)w * Q + q0 + P->hs_na[j] + u / 2;
+            const uint32_t c = P->hp_col_b[b0 + u];
+            if (q0 + P->hs_na[j] + u / 2 < kMaxOpSlots)
+              dword(w, q0 + P->hs_na[j] + u / 2, u & 1) = colword(c & 0xffffu) | colword(c >> 16) << 16;
+            for (int l = 0; l < 32; ++l)
+              for (int x = 0; x < 2; ++x)
+                P->hs_val[(slot * 32 + l) * 4 + 2 * (u & 1) + x] = P->hp_val_b[((size_t)(b0 + u) * 32 + l) * 2 + x];
+          }
+        }
+        q0 += P->hs_na[j] + P->hs_nb[j];
+      }
+    }
+  }
+  if (o.global_mode == 3 && P->hs_slots > kMaxOpSlots)
+    o.global_mode = 2;   // more slots per warp than the descriptor registers hold: 3xTF32 blocks
+  // default: the fp16-split streams where they apply (measured 7 % faster per step than 3xTF32 on
+  // config 4), else the 3xTF32 blocks
+  P->global_mode = o.global_mode ? o.global_mode : (P->hs_slots <= kMaxOpSlots ? 3 : 2);
   o.cells_per_cta = k;
   o.global_mode = P->global_mode;
   P->opt = o;

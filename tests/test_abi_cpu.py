@@ -114,6 +114,39 @@ def test_single_tf32_blocks_stay_below_fp32_rounding_of_the_row_sum(cell):
         assert info["n_op_blocks_tf32x1"] > info["n_op_blocks"] // 4
 
 
+def test_fp16_split_operator_is_fp32_equivalent_and_its_single_product_tier_is_bounded(cell):
+    """global_mode 3 stores every kept block as hi = fp16(x 2^k), lo = fp16(x 2^k - hi) with a power-of-
+    two row scaling: hi + lo must reproduce the fp32 operator to 2^-23 of the row's largest entry
+    (rows sit in [2^13, 2^14), fp16 resolves 2^-24 absolute there).  Blocks applied as ONE product
+    of the hi parts (error <= 2^-11 per product: both operands rounded to 11 bits) may hold at most
+    2^-13 of any row's l1 mass, so their total error stays below 2^-24 ||row||_1 |r|_max."""
+    rest, tris, mat, plan, oc = cell
+    n = rest.shape[0]
+    info = plan.info()
+    op = plan.query("operator").reshape(n, n)
+    f16 = plan.query("operator_f16").reshape(n, n)
+    x1 = plan.query("operator_f16x1").reshape(n, n)
+    rowmax = np.abs(op).max(axis=1, keepdims=True)
+    assert np.array_equal(f16 != 0, op != 0) or (np.abs(op[(f16 != 0) != (op != 0)]) <= rowmax.max() * 2.0 ** -37).all()
+    full = x1 == 0                                                      # three-product blocks: hi + lo
+    assert (np.abs(f16 - op)[full] <= (2.0 ** -23 * rowmax * np.ones_like(op))[full]).all()
+    single = x1 != 0                                                    # one-product blocks: hi alone
+    assert (np.abs(f16 - op)[single] <= (2.0 ** -11 * np.abs(op) + 2.0 ** -37 * rowmax)[single]).all()
+    assert np.array_equal(x1[single], f16[single])
+    assert (np.diag(x1) == 0).all()                                     # never the diagonal blocks
+    assert 0 <= info["n_op_blocks_f16x1"] < info["n_op_blocks"]
+    share = np.abs(np.where(single, op, 0.0)).sum(axis=1) / np.abs(op).sum(axis=1)
+    assert share.max() <= 2.0 ** -13 * (1 + 1e-6)
+    if n >= 600:                                                        # RBC-3: the tier is really used
+        assert info["n_op_blocks_f16x1"] > info["n_op_blocks_tf32x1"]
+    # the hi parts are fp16 numbers: the library's rounding agrees with numpy's float16
+    k = np.round(np.log2(rowmax / np.abs(f16).max(axis=1, keepdims=True)))  # 0: same scaling both sides
+    assert (k == 0).all()
+    scale = 2.0 ** (13 - np.floor(np.log2(rowmax)))
+    hi_np = (op * scale).astype(np.float32).astype(np.float16).astype(np.float64) / scale
+    assert np.array_equal(x1[single], hi_np[single])
+
+
 def test_elements_pair_all_triangles_of_the_icospheres(cell):
     """The local step works on elements = pairs of triangles across a shared edge (a matching of
     the dual graph); on the icospheres the matching is perfect, so E = T/2 threads do the work."""

@@ -73,8 +73,8 @@ def test_cells_per_cta_variants_and_ragged_tails(k):
     _parity(_G(rest, tris, mat, pos0, vel0), forces, 6, cells_per_cta=k)
 
 
-@pytest.mark.parametrize("mode", [1, 2])
-def test_global_step_modes_simt_and_3xtf32(mode):
+@pytest.mark.parametrize("mode", [1, 2, 3])
+def test_global_step_modes_simt_3xtf32_and_fp16_split(mode):
     rest, tris, mat, pos0, vel0, forces = _small_workload(level=3, n_cells=6)
     _parity(_G(rest, tris, mat, pos0, vel0), forces, 8, global_mode=mode)
 
