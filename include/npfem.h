@@ -266,6 +266,11 @@ int npfem_plan_info(npfem_plan p, npfem_info* out);
                               /* row scaling undone) expanded to a dense matrix in caller order;   */
                               /* one-product blocks contribute their hi part only                  */
 #define NPFEM_Q_OPERATOR_F16X1 12 /* double [n_verts^2]: only the blocks applied as one fp16 product */
+#define NPFEM_Q_OPERATOR_STREAM 13 /* double [n_verts^2]: the same operator as NPFEM_Q_OPERATOR_F16, but  */
+                              /* read back from the per-warp streams the kernel consumes (slot order,  */
+                              /* descriptors, row table): every kept block exactly once                */
+#define NPFEM_Q_STREAM_SHAPE 14 /* int32 [10]: warps, slots per warp, three-product slots of row slots  */
+                              /* 0..3, one-product slots of row slots 0..3                             */
 int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems);
 
 #ifdef __cplusplus

@@ -234,6 +234,55 @@ int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems) {
         }
       return (int)elems;
     }
+    case NPFEM_Q_STREAM_SHAPE: {
+      int32_t shape[10] = {P.threads / 32, P.hs_slots, P.hs_na[0], P.hs_na[1], P.hs_na[2], P.hs_na[3],
+                           P.hs_nb[0], P.hs_nb[1], P.hs_nb[2], P.hs_nb[3]};
+      return copy_out(shape, 10, sizeof(int32_t));
+    }
+    case NPFEM_Q_OPERATOR_STREAM: {
+      // walk the streams exactly as the kernel does: warp w, row slot j, first hs_na[j] three-product
+      // slots (one pair: words 0,1 hi, 2,3 lo), then hs_nb[j] one-product slots (two pairs: hi, hi)
+      const size_t elems = (size_t)n * n;
+      if (!dst) return (int)elems;
+      if ((size_t)dst_elems < elems) return set_err(NPFEM_EINVAL, "destination too small");
+      if (P.hs_slots > kMaxOpSlots) return set_err(NPFEM_EINVAL, "no streams: more slots per warp than the kernel supports");
+      double* D = static_cast<double*>(dst);
+      std::memset(D, 0, elems * sizeof(double));
+      auto hv = [](uint32_t w, int q) {
+        const uint32_t hb = (w >> (16 * q)) & 0xffffu;
+        const int e = (hb >> 10) & 0x1f, m = hb & 0x3ff;
+        const double v = e == 0 ? std::ldexp((double)m, -24) : std::ldexp((double)(m | 0x400), e - 25);
+        return (hb & 0x8000u) ? -v : v;
+      };
+      const int W = P.threads / 32, Q = P.hs_slots;
+      for (int w = 0; w < W; ++w) {
+        int q = 0;
+        for (int j = 0; j < 4; ++j) {
+          const int ib = P.hs_rows[(size_t)j * 32 + w];
+          for (int u = 0; u < P.hs_na[j] + P.hs_nb[j]; ++u, ++q) {
+            if (ib == 255) continue;
+            const bool full = u < P.hs_na[j];
+            for (int pr = 0; pr < (full ? 1 : 2); ++pr) {
+              const uint32_t dw = P.hs_desc[((size_t)w * 32 + (q & 31)) * 4 + 2 * ((q >> 5) & 1) + pr];
+              for (int l = 0; l < 32; ++l)
+                for (int half = 0; half < 2; ++half) {
+                  const uint32_t off = (dw >> (16 * half)) & 0xffffu;
+                  const int jb = (int)(off >> 9);
+                  if ((off & 0x1ffu) != ((uint32_t)(jb & 7) << 5)) return set_err(NPFEM_EINVAL, "internal: descriptor swizzle bits");
+                  const uint32_t* val = &P.hs_val[(((size_t)w * Q + q) * 32 + l) * 4];
+                  for (int e2 = 0; e2 < 2; ++e2) {
+                    const int i = ib * 8 + (l >> 2), jv = jb * 8 + 2 * (l & 3) + e2;
+                    if (i >= n || jv >= n) continue;
+                    double x = full ? hv(val[half], e2) + hv(val[2 + half], e2) : hv(val[2 * pr + half], e2);
+                    D[(size_t)P.perm[i] * n + P.perm[jv]] += x * (double)P.hp_scale[i];
+                  }
+                }
+            }
+          }
+        }
+      }
+      return (int)elems;
+    }
     default: return set_err(NPFEM_EINVAL, "unknown query");
   }
 }

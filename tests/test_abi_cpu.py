@@ -147,6 +147,73 @@ def test_fp16_split_operator_is_fp32_equivalent_and_its_single_product_tier_is_b
     assert np.array_equal(x1[single], hi_np[single])
 
 
+def test_operator_streams_hold_every_block_once_in_a_uniform_shape(cell):
+    """global_mode 3 consumes per-warp streams of 512-byte slots whose shape is the same for every
+    warp (per row slot j: na[j] three-product slots, nb[j] one-product slots).  Reading the streams
+    back the way the kernel walks them (slot order, descriptors with their swizzle bits, row table)
+    must give exactly the fp16 operator: no block lost, none twice, padding slots all zero."""
+    rest, tris, mat, plan, oc = cell
+    n = rest.shape[0]
+    info = plan.info()
+    shape = plan.query("stream_shape")
+    warps, slots, na, nb = int(shape[0]), int(shape[1]), shape[2:6], shape[6:10]
+    assert warps == info["threads_per_cta"] // 32
+    assert slots == int(na.sum() + nb.sum()) and 0 < slots <= 64
+    assert 4 * warps >= info["n_vblocks"]                               # at most 4 block rows per warp
+    stream = plan.query("operator_stream").reshape(n, n)
+    f16 = plan.query("operator_f16").reshape(n, n)
+    assert np.array_equal(stream, f16)
+    # work of the padded streams against the unpadded pair counts: the padding stays moderate
+    x1 = plan.query("operator_f16x1").reshape(n, n)
+    perm = plan.query("perm")
+    nvb = info["n_vblocks"]
+    def blocks(M):
+        Mp = np.zeros((nvb * 8, nvb * 8)); Mp[:n, :n] = M[np.ix_(perm, perm)]
+        return np.abs(Mp).reshape(nvb, 8, nvb, 8).sum(axis=(1, 3)) > 0
+    single = blocks(x1)
+    full = blocks(f16) & ~single
+    mma_needed = 3 * np.ceil(full.sum(axis=1) / 2).sum() + np.ceil(single.sum(axis=1) / 2).sum()
+    mma_issued = warps * (3 * na.sum() + 2 * nb.sum())
+    assert mma_needed <= mma_issued <= 1.6 * mma_needed + 12 * warps
+
+
+def test_fp16_split_product_emulated_in_numpy_is_fp32_equivalent(cell):
+    """The arithmetic of the global_mode-3 product, emulated on the CPU with numpy float16: right-
+    hand sides scaled per cell by a power of two to max |r| in [2^13, 2^14), split into hi = fp16(x),
+    lo = fp16(x - hi); operator rows scaled likewise; three products hi*hi + hi*lo + lo*hi for the
+    full-tier blocks, hi*hi for the single-tier blocks, fp32 accumulation.  Against T r in fp64 the
+    error must stay at the level of fp32 rounding of the row sums (a few 2^-24 ||row||_1 |r|_max)."""
+    rest, tris, mat, plan, oc = cell
+    n = rest.shape[0]
+    op = plan.query("operator").reshape(n, n)
+    x1 = plan.query("operator_f16x1").reshape(n, n)
+    single = x1 != 0
+    rowmax = np.abs(op).max(axis=1, keepdims=True)
+    tscale = 2.0 ** (13 - np.floor(np.log2(rowmax)))
+    ts = (op * tscale).astype(np.float32)
+    t_hi = ts.astype(np.float16)
+    t_lo = (ts - t_hi.astype(np.float32)).astype(np.float16)
+    rng = np.random.Generator(np.random.PCG64(11))
+    worst = 0.0
+    for trial in range(4):
+        r = (rng.standard_normal((n, 3)) * 10.0 ** rng.uniform(-6, 2)).astype(np.float32)
+        if trial == 3:
+            r[rng.random(n) < 0.5] *= 1e-5                               # wide dynamic range inside one cell
+        e = int(np.floor(np.log2(np.abs(r).max())))
+        rs = r * np.float32(2.0 ** (13 - e))
+        r_hi = rs.astype(np.float16)
+        r_lo = (rs - r_hi.astype(np.float32)).astype(np.float16)
+        th, tl = t_hi.astype(np.float64), np.where(single, 0.0, t_lo.astype(np.float64))
+        rh, rl = r_hi.astype(np.float64), r_lo.astype(np.float64)
+        full_mask = (~single).astype(np.float64)
+        acc = th @ rh + tl @ rh + (th * full_mask) @ rl                  # products exact in fp64; sums rounded below
+        got = acc.astype(np.float32).astype(np.float64) / tscale * 2.0 ** (e - 13)
+        want = op @ r.astype(np.float64)
+        bound = np.abs(op).sum(axis=1, keepdims=True) * np.abs(r).max()
+        worst = max(worst, float((np.abs(got - want) / bound).max()))
+    assert worst <= 4 * 2.0 ** -24
+
+
 def test_elements_pair_all_triangles_of_the_icospheres(cell):
     """The local step works on elements = pairs of triangles across a shared edge (a matching of
     the dual graph); on the icospheres the matching is perfect, so E = T/2 threads do the work."""
