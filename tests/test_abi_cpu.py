@@ -177,6 +177,23 @@ def test_operator_streams_hold_every_block_once_in_a_uniform_shape(cell):
     assert mma_needed <= mma_issued <= 1.6 * mma_needed + 12 * warps
 
 
+def test_global_mode_default_and_fallback():
+    """Default = the fp16-split streams (3); a plan whose streams would need more than 64 slots per
+    warp (here: the dense operator of RBC-3, 81 blocks in every row) falls back to 3xTF32 blocks (2),
+    also when mode 3 is asked for explicitly; modes 1 and 2 are honoured as given."""
+    rest, tris = W.rest_shape("rbc", 3)
+    mat = W.default_material(rest, tris)
+    assert NpfemPlan(tris, rest, mat, DT).info()["global_mode"] == 3
+    assert NpfemPlan(tris, rest, mat, DT, global_mode=2).info()["global_mode"] == 2
+    assert NpfemPlan(tris, rest, mat, DT, global_mode=1).info()["global_mode"] == 1
+    dense = NpfemPlan(tris, rest, mat, DT, inv_drop_tol=0.0)
+    assert dense.query("stream_shape")[1] > 64
+    assert dense.info()["global_mode"] == 2
+    assert NpfemPlan(tris, rest, mat, DT, inv_drop_tol=0.0, global_mode=3).info()["global_mode"] == 2
+    with pytest.raises(NpfemError):
+        dense.query("operator_stream")
+
+
 def test_fp16_split_product_emulated_in_numpy_is_fp32_equivalent(cell):
     """The arithmetic of the global_mode-3 product, emulated on the CPU with numpy float16: right-
     hand sides scaled per cell by a power of two to max |r| in [2^13, 2^14), split into hi = fp16(x),
