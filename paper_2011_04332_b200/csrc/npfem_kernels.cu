@@ -470,8 +470,13 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
         for (int q = 0; q < Q; q += kOpDepth) {
           uint4 rv[kOpDepth];
 #pragma unroll
-          for (int u = 0; u < kOpDepth; ++u)
+          for (int u = 0; u < kOpDepth; ++u) {
+            // the zero is never consumed (same guard below), but without it ptxas takes rv[] for
+            // live from the kernel's entry ("maybe uninitialised") and the ELEMENT PASS spills:
+            // 40 bytes of spill stores at kOpDepth 4, 0 with this line
+            rv[u] = make_uint4(0u, 0u, 0u, 0u);
             if (q + u < Q) rv[u] = ldg_stream(vp + (q + u) * 32);
+          }
 #pragma unroll
           for (int u = 0; u < kOpDepth; ++u) {
             if (q + u < Q) {
