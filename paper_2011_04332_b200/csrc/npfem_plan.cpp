@@ -390,6 +390,44 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
   // first, while their l1 mass stays <= 2^-15 of the l1 norm of EVERY row of the block row
   // (product error <= 2^-24 ||row||_1 |r|_max, the size of one fp32 rounding).  Each run is padded
   // with all-zero blocks to a multiple of 4 for the kernel's unrolled, software-pipelined loop.
+  auto Tint = [&](int i, int j) {   // operator entry in internal numbering, 0 outside
+    return (i < n && j < n) ? Tinv[(size_t)P->perm[i] * n + P->perm[j]] : 0.0;
+  };
+  // Kept source blocks of output block row ib (`cols`) and which of them may take the cheap single
+  // product (`single`): blocks are moved to that tier, smallest first (by their largest row mass),
+  // while the tier's l1 mass stays <= tier_tol of the l1 norm of EVERY row of the block row; the
+  // diagonal block never moves.
+  auto tier_split = [&](int ib, double tier_tol, std::vector<int>& cols, std::vector<uint8_t>& single) {
+    cols.clear();
+    for (int jb = 0; jb < nvb; ++jb)
+      if (bmask[(size_t)ib * nvb + jb]) cols.push_back(jb);
+    std::vector<std::array<double, 8>> mass(cols.size());
+    std::array<double, 8> rowl1{};
+    for (size_t q = 0; q < cols.size(); ++q)
+      for (int r = 0; r < 8; ++r) {
+        double m = 0.0;
+        for (int cc = 0; cc < 8; ++cc) m += std::fabs(Tint(ib * 8 + r, cols[q] * 8 + cc));
+        mass[q][r] = m;
+        rowl1[r] += m;
+      }
+    std::vector<int> order(cols.size());
+    std::iota(order.begin(), order.end(), 0);
+    auto bmax = [&](int q) { return *std::max_element(mass[q].begin(), mass[q].end()); };
+    std::sort(order.begin(), order.end(), [&](int p, int q) {
+      double mp = bmax(p), mq = bmax(q);
+      return mp != mq ? mp < mq : p < q;
+    });
+    single.assign(cols.size(), 0);
+    std::array<double, 8> cum{};
+    for (int q : order) {
+      bool ok = cols[q] != ib;
+      for (int r = 0; r < 8 && ok; ++r)
+        if (rowl1[r] > 0.0 && cum[r] + mass[q][r] > tier_tol * rowl1[r]) ok = false;
+      if (!ok) break;
+      for (int r = 0; r < 8; ++r) cum[r] += mass[q][r];
+      single[q] = 1;
+    }
+  };
   P->blk_ptr.assign(3 * (size_t)nvb, 0);
   P->blk_col.clear();
   P->blk_val.clear();
@@ -397,9 +435,6 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
   P->n_op_blocks_x1 = 0;
   {
     const double tier_tol = std::ldexp(1.0, -15);
-    auto Tint = [&](int i, int j) {   // operator entry in internal numbering, 0 outside
-      return (i < n && j < n) ? Tinv[(size_t)P->perm[i] * n + P->perm[j]] : 0.0;
-    };
     auto emit = [&](int ib, int jb, bool zero) {
       P->blk_col.push_back((uint16_t)jb);
       size_t base = P->blk_val.size();
@@ -414,35 +449,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     };
     for (int ib = 0; ib < nvb; ++ib) {
       std::vector<int> cols;
-      for (int jb = 0; jb < nvb; ++jb)
-        if (bmask[(size_t)ib * nvb + jb]) cols.push_back(jb);
-      // l1 mass of each kept block per row of the block row, and the rows' l1 norms over kept blocks
-      std::vector<std::array<double, 8>> mass(cols.size());
-      std::array<double, 8> rowl1{};
-      for (size_t q = 0; q < cols.size(); ++q)
-        for (int r = 0; r < 8; ++r) {
-          double m = 0.0;
-          for (int cc = 0; cc < 8; ++cc) m += std::fabs(Tint(ib * 8 + r, cols[q] * 8 + cc));
-          mass[q][r] = m;
-          rowl1[r] += m;
-        }
-      std::vector<int> order(cols.size());
-      std::iota(order.begin(), order.end(), 0);
-      auto bmax = [&](int q) { return *std::max_element(mass[q].begin(), mass[q].end()); };
-      std::sort(order.begin(), order.end(), [&](int p, int q) {
-        double mp = bmax(p), mq = bmax(q);
-        return mp != mq ? mp < mq : p < q;
-      });
-      std::vector<uint8_t> single(cols.size(), 0);
-      std::array<double, 8> cum{};
-      for (int q : order) {
-        bool ok = cols[q] != ib;   // the diagonal block always stays in the 3xTF32 run
-        for (int r = 0; r < 8 && ok; ++r)
-          if (rowl1[r] > 0.0 && cum[r] + mass[q][r] > tier_tol * rowl1[r]) ok = false;
-        if (!ok) break;
-        for (int r = 0; r < 8; ++r) cum[r] += mass[q][r];
-        single[q] = 1;
-      }
+      std::vector<uint8_t> single;
+      tier_split(ib, tier_tol, cols, single);
       for (int pass = 0; pass < 2; ++pass) {
         P->blk_ptr[3 * (size_t)ib + pass] = (int32_t)P->blk_col.size();
         int run_blocks = 0;
@@ -475,9 +483,6 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
   //      A run with an odd number of blocks ends with a half-empty pair.
   {
     const double tier_tol = std::ldexp(1.0, -13);
-    auto Tint = [&](int i, int j) {
-      return (i < n && j < n) ? Tinv[(size_t)P->perm[i] * n + P->perm[j]] : 0.0;
-    };
     std::vector<int> kexp(nvb * 8, 0);
     P->hp_scale.assign(n, 1.0f);
     for (int i = 0; i < n; ++i) {
@@ -520,34 +525,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     };
     for (int ib = 0; ib < nvb; ++ib) {
       std::vector<int> cols;
-      for (int jb = 0; jb < nvb; ++jb)
-        if (bmask[(size_t)ib * nvb + jb]) cols.push_back(jb);
-      std::vector<std::array<double, 8>> mass(cols.size());
-      std::array<double, 8> rowl1{};
-      for (size_t q = 0; q < cols.size(); ++q)
-        for (int r = 0; r < 8; ++r) {
-          double m = 0.0;
-          for (int cc = 0; cc < 8; ++cc) m += std::fabs(Tint(ib * 8 + r, cols[q] * 8 + cc));
-          mass[q][r] = m;
-          rowl1[r] += m;
-        }
-      std::vector<int> order(cols.size());
-      std::iota(order.begin(), order.end(), 0);
-      auto bmax = [&](int q) { return *std::max_element(mass[q].begin(), mass[q].end()); };
-      std::sort(order.begin(), order.end(), [&](int p, int q) {
-        double mp = bmax(p), mq = bmax(q);
-        return mp != mq ? mp < mq : p < q;
-      });
-      std::vector<uint8_t> single(cols.size(), 0);
-      std::array<double, 8> cum{};
-      for (int q : order) {
-        bool ok = cols[q] != ib;   // the diagonal block always takes three products
-        for (int r = 0; r < 8 && ok; ++r)
-          if (rowl1[r] > 0.0 && cum[r] + mass[q][r] > tier_tol * rowl1[r]) ok = false;
-        if (!ok) break;
-        for (int r = 0; r < 8; ++r) cum[r] += mass[q][r];
-        single[q] = 1;
-      }
+      std::vector<uint8_t> single;
+      tier_split(ib, tier_tol, cols, single);
       for (int pass = 0; pass < 2; ++pass) {
         std::vector<uint32_t>& colv = pass ? P->hp_col_b : P->hp_col_a;
         P->hp_ptr[4 * (size_t)ib + 2 * pass] = (int32_t)colv.size();
