@@ -440,11 +440,11 @@ __global__ void __launch_bounds__(MAXT, 1) npfem_step_kernel(const DevParams P) 
     const int g8 = lane_p >> 2, t4 = lane_p & 3;
     if constexpr (MODE == 3) {
       // the warp's operator stream: slots of 512 bytes of B fragments, consumed in order.  The
-      // stream has the same shape for every warp (per row slot
-      // j: hs_na[j] three-product slots, then hs_nb[j] one-product slots), so every branch below
-      // is uniform; the slot descriptors (<= 64 slots per warp) sit in four registers, lane l
-      // holding those of slots l and l + 32, and are broadcast by shuffle; a finished block row
-      // goes straight to the owners' hand-off buffer (rb is not read in this phase)
+      // stream has the same shape for every warp (per row slot j: hs_na[j] three-product slots,
+      // then hs_nb[j] one-product slots), so every branch below is uniform; the slot descriptors
+      // (<= 64 slots per warp) sit in four registers, lane l holding those of slots l and l + 32,
+      // and are broadcast by shuffle; a finished block row goes straight to the owners' hand-off
+      // buffer (rb is not read in this phase)
       const int Q = NPFEM_PDBG(16) ? 0 : P.hs_slots;
       const uint4* const vp = P.hs_val + (size_t)warp_p * Q * 32 + lane_p;
       // (x, y) slot lane, (z, w) slot lane + 32.  The identity shuffles re-home the four words from
