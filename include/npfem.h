@@ -212,7 +212,10 @@ int npfem_measure_fp32_peak(int variant, double* out_tflops);
  * step kernel accumulates per phase of an iteration (0 prologue, 1 first element pass, 2 cell
  * pipeline, 3 right-hand-side split, 4 operator product, 5 hand-off, 6 owner update), summed over
  * CTAs and iterations since the last reset.  Blocking.
- *   out16  host, receives 16 counters;  reset  non-zero: zero the counters after reading
+ *   out16  host, receives 16 counters;  reset  1..255: zero the counters after reading; >= 0x100:
+ *          nothing is read, the low byte becomes the ablation mask of the global_mode-3 operator
+ *          product for later launches (1 no mma, 2 no shared-memory operand loads, 16 skip the
+ *          product loop, 32 skip the right-hand-side split; results are then meaningless)
  */
 int npfem_debug_phase_clocks(unsigned long long* out16, int reset);
 
