@@ -65,6 +65,10 @@ typedef struct {
   double strain_hardening;       /* beta >= 0: strain-dependent strain weight k_strain (1 + beta d^2),  */
                                  /* d = clamp(sigma) - sigma (reading A-23: "a weight */
                                  /* and various parameters ... stiffer or softer"); 0 = constant weight */
+  double w_garea, ga_min, ga_max; /* global-area term (reading A-24): weight and band on the total      */
+                                 /* surface area A/A0.  Implemented in the ORACLE only (its closest-   */
+                                 /* point projection needs a Newton solve with the dense area Hessian); */
+                                 /* npfem_create rejects w_garea != 0 with NPFEM_EINVAL                 */
 } npfem_material;
 
 /* Tuning knobs that do not change what is computed beyond fp32 rounding.  Pass NULL for defaults. */

@@ -20,8 +20,11 @@
  *  - PAPER.md:60 ("with minor modifications of equation (2), one can readily simulate a
  *    viscoelastic material"), :145, :183 (parameters Calpha, Cbeta): Rayleigh damping
  *    f_d = -(c_alpha M + c_beta L_el) v, integrated implicitly (reading A-20).
+ *  - PAPER.md:181-183 ("a weight and various parameters"): strain-dependent
+ *    strain weight (reading A-23) and a global-area term, one constraint per cell on the total
+ *    surface area (reading A-24; ORACLE ONLY, the CUDA library rejects it); both off by default.
  * The paper prints none of the energies; every formula below is a READING listed in DESIGN.md
- * (A-1 ... A-20).  Agreement with the real npFEM code is
+ * (A-1 ... A-24).  Agreement with the real npFEM code is
  * "parity unpinned"; what IS pinned (tests/test_oracle_pins.py) are invariants, closed forms,
  * library routines and brute force.
  *
@@ -52,6 +55,7 @@ typedef struct {
   double c_alpha, c_beta;
   double w_collision, d_collision;   /* collision weight per vertex, contact distance (reading A-22) */
   double strain_hardening;           /* beta >= 0: strain-dependent weight w_s (1 + beta d^2) (reading A-23) */
+  double w_garea, ga_min, ga_max;    /* global-area term: weight, band on A/A0 of the whole surface (reading A-24) */
 } oracle_material;
 
 typedef struct oracle_cell {
@@ -351,6 +355,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   if (mat->s_min > mat->s_max || mat->a_min > mat->a_max || mat->v_min > mat->v_max) return ORACLE_EINVAL;
   if (mat->c_alpha < 0.0 || mat->c_beta < 0.0) return ORACLE_EINVAL;
   if (mat->w_collision < 0.0 || mat->d_collision < 0.0 || mat->strain_hardening < 0.0) return ORACLE_EINVAL;
+  if (mat->w_garea < 0.0 || (mat->w_garea > 0.0 && mat->ga_min > mat->ga_max)) return ORACLE_EINVAL;
   if (!(mat->cell_mass > 0)) return ORACLE_EINVAL;
   for (int i = 0; i < 3*T; ++i) if (tris[i] < 0 || tris[i] >= n) return ORACLE_EINVAL;
   if ((3*T) % 2) return ORACLE_EINVAL;
@@ -451,7 +456,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   if (!(c->V0 > 0)) { oracle_destroy(c); return ORACLE_EINVAL; }
 
   /* step 5: L_el = sum_t (w_s+w_a) G^T G + sum_h w_h K^T K;
-   *         A_sys = (1/h^2 + c_alpha/h) diag(m) + (1 + c_beta/h) L_el + (w_volume + w_collision) I
+   *         A_sys = (1/h^2 + c_alpha/h) diag(m) + (1 + c_beta/h) L_el + (w_volume + w_collision + w_garea) I
    * (c_alpha = c_beta = 0: the undamped system of SURVEY.md 8(c); otherwise reading A-20: the
    * Rayleigh damping force -(c_alpha M + c_beta L_el)(x - x_n)/h of implicit Euler moves
    * (c_alpha M + c_beta L_el)/h to the left-hand side) */
@@ -470,7 +475,7 @@ int oracle_create(int n, int T, const int32_t *tris, const double *X, const orac
   }
   for (size_t i = 0; i < (size_t)n*n; ++i) c->A[i] = (1.0 + mat->c_beta / h) * c->Lel[i];
   for (int v = 0; v < n; ++v)
-    c->A[(size_t)v*n+v] += c->mass[v] * (1.0/(h*h) + mat->c_alpha / h) + mat->w_volume + mat->w_collision;
+    c->A[(size_t)v*n+v] += c->mass[v] * (1.0/(h*h) + mat->c_alpha / h) + mat->w_volume + mat->w_collision + mat->w_garea;
   if (chol_dense(n, c->A, c->L) != 0) { oracle_destroy(c); return ORACLE_EINVAL; }
   for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) c->LT[(size_t)j*n+i] = c->L[(size_t)i*n+j];
   *out = c;
@@ -607,6 +612,8 @@ double oracle_energy(const oracle_cell *c, const double *x, const double *s, con
   return e[0] + e[1] + e[2] + e[3] + e[4];
 }
 
+double oracle_garea_local(const oracle_cell *c, const double *x, double *Pg);
+
 /* internal force f_int(x) = sum w A^T (p(x) - A x)   (pins P-2, P-8) */
 void oracle_fint(const oracle_cell *c, const double *x, double *f) {
   int n = c->n; const oracle_material *m = &c->mat;
@@ -622,12 +629,174 @@ void oracle_fint(const oracle_cell *c, const double *x, double *f) {
       for (int j = 0; j < n; ++j) s += c->Lel[(size_t)i*n+j] * x[3*j+d];
       f[3*i+d] -= s;
     }
-  (void)m;
+  if (m->w_garea > 0.0) {                                /* global-area term (A-24): w_garea (P_g - x) */
+    oracle_garea_local(c, x, zero);
+    for (size_t i = 0; i < 3*(size_t)n; ++i) f[i] += m->w_garea * (zero[i] - x[i]);
+  }
   free(Ps); free(Pa); free(Pb); free(Pv); free(zero);
 }
 
 void oracle_damping_rhs(const oracle_cell *c, const double *xn, double *b);
 double oracle_dissipation(const oracle_cell *c, const double *x, const double *xn);
+
+/* ---------------------------------------------------------------- global-area term (NEXT-4, reading A-24)
+ * every elemental potential has "a weight and various parameters"; SURVEY.md 8(f)
+ * NEXT-4 names "a global-area term".  Reading: one constraint per cell on the TOTAL surface area
+ * A(x) = sum_t 1/2 |(x_b - x_a) x (x_c - x_a)|, band [ga_min, ga_max] A0 (A0 = rest total area);
+ * P_g = the configuration closest to x (plain Euclidean norm over all 3n coordinates) with
+ * A(P_g) = A*; energy 1/2 w_garea ||x - P_g||^2 with selection matrix I, so w_garea sits on the
+ * diagonal of A_sys.  Unlike the volume, the area's Hessian (a cotangent Laplacian, entries of
+ * order 1) makes the fixed-point iteration D <- ((g.D - C)/(g.g)) g diverge already at a 10 %
+ * violation, so the closest point is found by Newton's method on the KKT system
+ *     P - x - lambda grad A(P) = 0,   A(P) = A*,
+ * Jacobian [[I - lambda H(P), -g], [g^T, 0]], H = Hessian of A, dense LU, step halving on the
+ * residual norm.  grad A: per triangle with unit normal nh, dA/dx_a = 1/2 nh x (x_c - x_b) (cyclic). */
+double oracle_area_total(int T, const int32_t *tris, const double *x) {
+  double A = 0.0;
+  for (int t = 0; t < T; ++t) {
+    const double *a = x + 3*tris[3*t], *b = x + 3*tris[3*t+1], *c = x + 3*tris[3*t+2];
+    double e1[3] = {b[0]-a[0], b[1]-a[1], b[2]-a[2]}, e2[3] = {c[0]-a[0], c[1]-a[1], c[2]-a[2]}, nn[3];
+    cross3(e1, e2, nn);
+    A += 0.5 * sqrt(dot3(nn, nn));
+  }
+  return A;
+}
+void oracle_area_grad(int n, int T, const int32_t *tris, const double *x, double *g) {
+  memset(g, 0, sizeof(double) * 3 * (size_t)n);
+  for (int t = 0; t < T; ++t) {
+    int id[3] = {tris[3*t], tris[3*t+1], tris[3*t+2]};
+    const double *a = x + 3*id[0], *b = x + 3*id[1], *c = x + 3*id[2];
+    double e1[3] = {b[0]-a[0], b[1]-a[1], b[2]-a[2]}, e2[3] = {c[0]-a[0], c[1]-a[1], c[2]-a[2]}, nn[3];
+    cross3(e1, e2, nn);
+    double len = sqrt(dot3(nn, nn));
+    if (!(len > 0.0)) continue;                          /* collapsed triangle: no contribution */
+    for (int k = 0; k < 3; ++k) nn[k] /= len;
+    for (int v = 0; v < 3; ++v) {                         /* opposite edge of vertex v: x_{v+2} - x_{v+1} */
+      const double *p = x + 3*id[(v+1)%3], *q = x + 3*id[(v+2)%3];
+      double opp[3] = {q[0]-p[0], q[1]-p[1], q[2]-p[2]}, gv[3];
+      cross3(nn, opp, gv);
+      for (int k = 0; k < 3; ++k) g[3*id[v]+k] += 0.5 * gv[k];
+    }
+  }
+}
+/* Hessian of the total area, dense [3n][3n].  Per triangle with u = b - a, v = c - a, n = u x v:
+ *   d n = J delta, J = [ -(e_k x v) - (u x e_k) | e_k x v | u x e_k ]  (3 x 9, columns a, b, c),
+ *   d^2 A = [ |J delta|^2 - (nh . J delta)^2 ] / (2 |n|) + nh . (du x dv),
+ * the last term being the quadratic form of 1/2 (X + X^T), X = S_v^T [nh]_x S_u, S_u = [-I I 0],
+ * S_v = [-I 0 I]. */
+void oracle_area_hessian(int n, int T, const int32_t *tris, const double *x, double *H) {
+  size_t m = 3 * (size_t)n;
+  memset(H, 0, sizeof(double) * m * m);
+  for (int t = 0; t < T; ++t) {
+    int id[3] = {tris[3*t], tris[3*t+1], tris[3*t+2]};
+    const double *a = x + 3*id[0], *b = x + 3*id[1], *c = x + 3*id[2];
+    double u[3] = {b[0]-a[0], b[1]-a[1], b[2]-a[2]}, v[3] = {c[0]-a[0], c[1]-a[1], c[2]-a[2]}, nn[3];
+    cross3(u, v, nn);
+    double len = sqrt(dot3(nn, nn));
+    if (!(len > 0.0)) continue;
+    double nh[3] = {nn[0]/len, nn[1]/len, nn[2]/len};
+    double J[3][9], Jn[9];
+    for (int k = 0; k < 3; ++k) {
+      double e[3] = {0, 0, 0}, ev[3], ue[3];
+      e[k] = 1.0;
+      cross3(e, v, ev); cross3(u, e, ue);
+      for (int r = 0; r < 3; ++r) { J[r][k] = -ev[r] - ue[r]; J[r][3+k] = ev[r]; J[r][6+k] = ue[r]; }
+    }
+    for (int q = 0; q < 9; ++q) Jn[q] = nh[0]*J[0][q] + nh[1]*J[1][q] + nh[2]*J[2][q];
+    /* [nh]_x y = nh x y */
+    double N[3][3] = {{0, -nh[2], nh[1]}, {nh[2], 0, -nh[0]}, {-nh[1], nh[0], 0}};
+    double Su[3][9] = {{0}}, Sv[3][9] = {{0}};
+    for (int k = 0; k < 3; ++k) { Su[k][k] = -1; Su[k][3+k] = 1; Sv[k][k] = -1; Sv[k][6+k] = 1; }
+    for (int p = 0; p < 9; ++p)
+      for (int q = 0; q < 9; ++q) {
+        double jj = J[0][p]*J[0][q] + J[1][p]*J[1][q] + J[2][p]*J[2][q];
+        double h = (jj - Jn[p]*Jn[q]) / (2.0 * len);
+        double X = 0, Xt = 0;                            /* X[p][q] = sum_rs Sv[r][p] N[r][s] Su[s][q] */
+        for (int r = 0; r < 3; ++r)
+          for (int ss = 0; ss < 3; ++ss) { X += Sv[r][p]*N[r][ss]*Su[ss][q]; Xt += Sv[r][q]*N[r][ss]*Su[ss][p]; }
+        h += 0.5 * (X + Xt);
+        H[(3*(size_t)id[p/3] + p%3) * m + 3*(size_t)id[q/3] + q%3] += h;
+      }
+  }
+}
+/* dense LU with partial pivoting: solves M y = rhs in place (M [m][m] is destroyed); 0 on success */
+static int lu_solve(int m, double *M, double *rhs) {
+  for (int k = 0; k < m; ++k) {
+    int piv = k; double best = fabs(M[(size_t)k*m+k]);
+    for (int i = k+1; i < m; ++i) if (fabs(M[(size_t)i*m+k]) > best) { best = fabs(M[(size_t)i*m+k]); piv = i; }
+    if (!(best > 0.0)) return -1;
+    if (piv != k) {
+      for (int j = 0; j < m; ++j) { double tmp = M[(size_t)k*m+j]; M[(size_t)k*m+j] = M[(size_t)piv*m+j]; M[(size_t)piv*m+j] = tmp; }
+      double tmp = rhs[k]; rhs[k] = rhs[piv]; rhs[piv] = tmp;
+    }
+    for (int i = k+1; i < m; ++i) {
+      double f = M[(size_t)i*m+k] / M[(size_t)k*m+k];
+      if (f == 0.0) continue;
+      for (int j = k+1; j < m; ++j) M[(size_t)i*m+j] -= f * M[(size_t)k*m+j];
+      rhs[i] -= f * rhs[k];
+    }
+  }
+  for (int i = m-1; i >= 0; --i) {
+    double s = rhs[i];
+    for (int j = i+1; j < m; ++j) s -= M[(size_t)i*m+j] * rhs[j];
+    rhs[i] = s / M[(size_t)i*m+i];
+  }
+  return 0;
+}
+/* closest configuration with total area Astar; returns the Newton iterations used (-1: no convergence) */
+int oracle_project_garea(int n, int T, const int32_t *tris, const double *x, double Astar, double A0,
+                         double *P) {
+  size_t m = 3 * (size_t)n; int mm = (int)m + 1;
+  memcpy(P, x, m * sizeof(double));
+  if (oracle_area_total(T, tris, x) == Astar) return 0;
+  double *g = (double*)malloc(m * sizeof(double)), *H = (double*)malloc(m * m * sizeof(double));
+  double *K = (double*)malloc((size_t)mm * mm * sizeof(double)), *rhs = (double*)malloc(mm * sizeof(double));
+  double *Pt = (double*)malloc(m * sizeof(double));
+  double lam = 0.0, scale = 0.0;
+  for (size_t i = 0; i < m; ++i) { double x0 = x[i] - x[i % 3]; scale += x0*x0; }
+  scale = sqrt(scale);                                   /* size of the cell, not its distance from the origin */
+  int it, ok = -1;
+  for (it = 1; it <= 60; ++it) {
+    oracle_area_grad(n, T, tris, P, g);
+    double C = oracle_area_total(T, tris, P) - Astar, r1n = 0;
+    for (size_t i = 0; i < m; ++i) { rhs[i] = -(P[i] - x[i] - lam * g[i]); r1n += rhs[i]*rhs[i]; }
+    rhs[m] = -C;
+    double res = sqrt(r1n) / scale + fabs(C) / fabs(A0);
+    if (res < 1e-14) { ok = it - 1; break; }
+    oracle_area_hessian(n, T, tris, P, H);
+    for (size_t i = 0; i < m; ++i) {
+      for (size_t j = 0; j < m; ++j) K[i*mm+j] = (i == j ? 1.0 : 0.0) - lam * H[i*m+j];
+      K[i*mm+m] = -g[i];
+      K[m*mm+i] = g[i];
+    }
+    K[m*mm+m] = 0.0;
+    if (lu_solve(mm, K, rhs) != 0) break;
+    double step = 1.0;                                   /* halve the step while the residual grows */
+    for (int ls = 0; ls < 30; ++ls, step *= 0.5) {
+      for (size_t i = 0; i < m; ++i) Pt[i] = P[i] + step * rhs[i];
+      double lt = lam + step * rhs[m];
+      oracle_area_grad(n, T, tris, Pt, g);
+      double Ct = oracle_area_total(T, tris, Pt) - Astar, rn = 0;
+      for (size_t i = 0; i < m; ++i) { double q = Pt[i] - x[i] - lt * g[i]; rn += q*q; }
+      if (sqrt(rn) / scale + fabs(Ct) / fabs(A0) < res || ls == 29) { memcpy(P, Pt, m * sizeof(double)); lam = lt; break; }
+    }
+  }
+  free(g); free(H); free(K); free(rhs); free(Pt);
+  return ok;
+}
+double oracle_rest_area(const oracle_cell *c) { double A = 0; for (int t = 0; t < c->T; ++t) A += c->area[t]; return A; }
+/* P_g [n][3] at x; returns the energy 1/2 w_garea ||x - P_g||^2 (0 and P_g = x when the weight is 0) */
+double oracle_garea_local(const oracle_cell *c, const double *x, double *Pg) {
+  size_t m3 = 3*(size_t)c->n;
+  if (!(c->mat.w_garea > 0.0)) { memcpy(Pg, x, sizeof(double)*m3); return 0.0; }
+  double A0 = oracle_rest_area(c);
+  double A = oracle_area_total(c->T, c->tris, x);
+  double Astar = clampd(A, c->mat.ga_min * A0, c->mat.ga_max * A0);
+  oracle_project_garea(c->n, c->T, c->tris, x, Astar, A0, Pg);
+  double e = 0;
+  for (size_t i = 0; i < m3; ++i) e += (x[i]-Pg[i])*(x[i]-Pg[i]);
+  return 0.5 * c->mat.w_garea * e;
+}
 
 /* ---------------------------------------------------------------- collisions (NEXT-3, reading A-22)
  * the coupling hands "external forces & colliding neighbours" to the solid solver;
@@ -661,9 +830,10 @@ double oracle_collision_local(const oracle_cell *c, const double *x, const doubl
 void oracle_step_cell_collide(const oracle_cell *c, double *pos, double *vel, const double *fext,
                               const double *q, const double *nrm, int n_iters, double *iterates,
                               double *energies) {
-  int n = c->n; size_t m3 = 3*(size_t)n; double h = c->h, wc = c->mat.w_collision;
+  int n = c->n; size_t m3 = 3*(size_t)n; double h = c->h, wc = c->mat.w_collision, wg = c->mat.w_garea;
   double *s = (double*)malloc(sizeof(double)*m3), *x = (double*)malloc(sizeof(double)*m3);
   double *b = (double*)malloc(sizeof(double)*m3), *Pc = (double*)malloc(sizeof(double)*m3);
+  double *Pg = wg > 0.0 ? (double*)malloc(sizeof(double)*m3) : NULL;   /* global-area term (A-24), off by default */
   double *Ps = (double*)malloc(sizeof(double)*6*c->T), *Pa = (double*)malloc(sizeof(double)*6*c->T);
   double *Pb = (double*)malloc(sizeof(double)*3*c->H), *Pv = (double*)malloc(sizeof(double)*m3);
   for (int v = 0; v < n; ++v)
@@ -674,20 +844,23 @@ void oracle_step_cell_collide(const oracle_cell *c, double *pos, double *vel, co
   for (int k = 0; k < n_iters; ++k) {
     oracle_local(c, x, Ps, Pa, Pb, Pv);
     double ec = oracle_collision_local(c, x, q, nrm, Pc);
-    if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + ec;
+    double eg = Pg ? oracle_garea_local(c, x, Pg) : 0.0;
+    if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + ec + eg;
     oracle_rhs(c, s, Ps, Pa, Pb, Pv, b);
     oracle_damping_rhs(c, pos, b);
     for (size_t i = 0; i < m3; ++i) b[i] += wc * Pc[i];
+    if (Pg) for (size_t i = 0; i < m3; ++i) b[i] += wg * Pg[i];
     oracle_solve(c, b, x);
     if (energies) {
-      double e2 = 0;
+      double e2 = 0, e3 = 0;
       for (size_t i = 0; i < m3; ++i) e2 += (x[i]-Pc[i])*(x[i]-Pc[i]);
-      energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + 0.5*wc*e2;
+      if (Pg) for (size_t i = 0; i < m3; ++i) e3 += (x[i]-Pg[i])*(x[i]-Pg[i]);
+      energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + 0.5*wc*e2 + 0.5*wg*e3;
     }
     if (iterates) memcpy(iterates + (size_t)(k+1)*m3, x, sizeof(double)*m3);
   }
   for (size_t i = 0; i < m3; ++i) { vel[i] = (x[i] - pos[i]) / h; pos[i] = x[i]; }
-  free(s); free(x); free(b); free(Pc); free(Ps); free(Pa); free(Pb); free(Pv);
+  free(s); free(x); free(b); free(Pc); free(Pg); free(Ps); free(Pa); free(Pb); free(Pv);
 }
 void oracle_step_collide(const oracle_cell *c, int n_cells, double *pos, double *vel, const double *fext,
                          const double *q, const double *nrm, int n_iters) {
@@ -749,11 +922,12 @@ double oracle_dissipation(const oracle_cell *c, const double *x, const double *x
  * energies [2*n_iters]: E(x^k;p^k) after each local step, E(x^{k+1};p^k) after each global step. */
 void oracle_step_cell(const oracle_cell *c, double *pos, double *vel, const double *fext,
                       int n_iters, double *iterates, double *energies) {
-  int n = c->n; size_t m3 = 3*(size_t)n; double h = c->h;
+  int n = c->n; size_t m3 = 3*(size_t)n; double h = c->h, wg = c->mat.w_garea;
   double *s = (double*)malloc(sizeof(double)*m3), *x = (double*)malloc(sizeof(double)*m3);
   double *b = (double*)malloc(sizeof(double)*m3);
   double *Ps = (double*)malloc(sizeof(double)*6*c->T), *Pa = (double*)malloc(sizeof(double)*6*c->T);
   double *Pb = (double*)malloc(sizeof(double)*3*c->H), *Pv = (double*)malloc(sizeof(double)*m3);
+  double *Pg = wg > 0.0 ? (double*)malloc(sizeof(double)*m3) : NULL;   /* global-area term (A-24), off by default */
   for (int v = 0; v < n; ++v)
     for (int d = 0; d < 3; ++d)
       s[3*v+d] = pos[3*v+d] + h * vel[3*v+d] + h*h * fext[3*v+d] / c->mass[v];
@@ -761,15 +935,26 @@ void oracle_step_cell(const oracle_cell *c, double *pos, double *vel, const doub
   if (iterates) memcpy(iterates, x, sizeof(double)*m3);
   for (int k = 0; k < n_iters; ++k) {
     oracle_local(c, x, Ps, Pa, Pb, Pv);
-    if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos);
-    oracle_rhs(c, s, Ps, Pa, Pb, Pv, b);
-    oracle_damping_rhs(c, pos, b);
-    oracle_solve(c, b, x);
-    if (energies) energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos);
+    if (!Pg) {                                             /* the path of the five configs, untouched */
+      if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos);
+      oracle_rhs(c, s, Ps, Pa, Pb, Pv, b);
+      oracle_damping_rhs(c, pos, b);
+      oracle_solve(c, b, x);
+      if (energies) energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos);
+    } else {
+      double eg = oracle_garea_local(c, x, Pg), e3 = 0;
+      if (energies) energies[2*k] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + eg;
+      oracle_rhs(c, s, Ps, Pa, Pb, Pv, b);
+      oracle_damping_rhs(c, pos, b);
+      for (size_t i = 0; i < m3; ++i) b[i] += wg * Pg[i];
+      oracle_solve(c, b, x);
+      for (size_t i = 0; i < m3; ++i) e3 += (x[i]-Pg[i])*(x[i]-Pg[i]);
+      if (energies) energies[2*k+1] = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, pos) + 0.5*wg*e3;
+    }
     if (iterates) memcpy(iterates + (size_t)(k+1)*m3, x, sizeof(double)*m3);
   }
   for (size_t i = 0; i < m3; ++i) { vel[i] = (x[i] - pos[i]) / h; pos[i] = x[i]; }
-  free(s); free(x); free(b); free(Ps); free(Pa); free(Pb); free(Pv);
+  free(s); free(x); free(b); free(Ps); free(Pa); free(Pb); free(Pv); free(Pg);
 }
 
 /* ---------------------------------------------------------------- converged solve (NEXT-1)
@@ -795,6 +980,7 @@ double oracle_objective(const oracle_cell *c, const double *x, const double *s, 
   double *Pb = (double*)malloc(sizeof(double)*3*c->H), *Pv = (double*)malloc(sizeof(double)*m3);
   oracle_local(c, x, Ps, Pa, Pb, Pv);
   double gval = oracle_energy(c, x, s, Ps, Pa, Pb, Pv, NULL) + oracle_dissipation(c, x, xn);
+  if (c->mat.w_garea > 0.0) gval += oracle_garea_local(c, x, Pv);   /* Pv is free again: global-area energy (A-24) */
   if (grad) {
     double *f = (double*)malloc(sizeof(double)*m3), *dmp = (double*)calloc(m3, sizeof(double));
     oracle_fint(c, x, f);

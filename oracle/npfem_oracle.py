@@ -16,7 +16,7 @@ from . import build as _build
 
 MATERIAL_FIELDS = ("cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min", "a_max",
                    "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta", "w_collision",
-                   "d_collision", "strain_hardening")
+                   "d_collision", "strain_hardening", "w_garea", "ga_min", "ga_max")
 
 
 class _Material(C.Structure):
@@ -59,6 +59,16 @@ def lib():
         L.oracle_volume_grad.argtypes = [C.c_int, C.c_int, _ip, _dp, _dp]
         L.oracle_project_volume.restype = C.c_int
         L.oracle_project_volume.argtypes = [C.c_int, C.c_int, _ip, _dp, C.c_double, C.c_double, _dp]
+        L.oracle_area_total.restype = C.c_double
+        L.oracle_area_total.argtypes = [C.c_int, _ip, _dp]
+        L.oracle_area_grad.argtypes = [C.c_int, C.c_int, _ip, _dp, _dp]
+        L.oracle_area_hessian.argtypes = [C.c_int, C.c_int, _ip, _dp, _dp]
+        L.oracle_project_garea.restype = C.c_int
+        L.oracle_project_garea.argtypes = [C.c_int, C.c_int, _ip, _dp, C.c_double, C.c_double, _dp]
+        L.oracle_rest_area.restype = C.c_double
+        L.oracle_rest_area.argtypes = [C.c_void_p]
+        L.oracle_garea_local.restype = C.c_double
+        L.oracle_garea_local.argtypes = [C.c_void_p, _dp, _dp]
         L.oracle_deformation_gradient.argtypes = [C.c_void_p, C.c_int, _dp, _dp]
         L.oracle_local.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
         L.oracle_rhs.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp, _dp]
@@ -161,6 +171,35 @@ def project_volume(tris, x, v_star, v0):
     P = np.empty_like(x)
     its = lib().oracle_project_volume(x.shape[0], tris.shape[0], _i(tris), _d(x), float(v_star),
                                       float(v0), _d(P))
+    return P, int(its)
+
+
+def area_total(tris, x):
+    """Total surface area (global-area term, reading A-24)."""
+    tris = np.ascontiguousarray(tris, dtype=np.int32); x = _f64(x)
+    return float(lib().oracle_area_total(tris.shape[0], _i(tris), _d(x)))
+
+
+def area_grad(tris, x):
+    tris = np.ascontiguousarray(tris, dtype=np.int32); x = _f64(x)
+    g = np.empty_like(x)
+    lib().oracle_area_grad(x.shape[0], tris.shape[0], _i(tris), _d(x), _d(g))
+    return g
+
+
+def area_hessian(tris, x):
+    tris = np.ascontiguousarray(tris, dtype=np.int32); x = _f64(x)
+    H = np.empty((3 * x.shape[0], 3 * x.shape[0]))
+    lib().oracle_area_hessian(x.shape[0], tris.shape[0], _i(tris), _d(x), _d(H))
+    return H
+
+
+def project_garea(tris, x, a_star, a0):
+    """Closest configuration with total area a_star (Newton on the KKT system); (P, iterations)."""
+    tris = np.ascontiguousarray(tris, dtype=np.int32); x = _f64(x)
+    P = np.empty_like(x)
+    its = lib().oracle_project_garea(x.shape[0], tris.shape[0], _i(tris), _d(x), float(a_star),
+                                     float(a0), _d(P))
     return P, int(its)
 
 
@@ -293,6 +332,15 @@ class OracleCell:
         lib().oracle_step_collide(self._h, pos.shape[0], _d(pos), _d(vel), _d(fext), _d(q), _d(nrm),
                                   int(n_iters))
         return pos, vel
+
+    def rest_area(self):
+        return float(lib().oracle_rest_area(self._h))
+
+    def garea_local(self, x):
+        """(P_g, energy) of the global-area term at x (reading A-24); P_g = x, 0 when w_garea = 0."""
+        x = _f64(x); P = np.empty_like(x)
+        e = float(lib().oracle_garea_local(self._h, _d(x), _d(P)))
+        return P, e
 
     def vertex_areas(self, x):
         x = _f64(x); a = np.empty(self.n)

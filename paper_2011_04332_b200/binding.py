@@ -14,7 +14,7 @@ from . import build as _build
 
 MATERIAL_FIELDS = ("cell_mass", "k_strain", "s_min", "s_max", "k_area", "a_min", "a_max",
                    "k_bend", "w_volume", "v_min", "v_max", "c_alpha", "c_beta", "w_collision",
-                   "d_collision", "strain_hardening")
+                   "d_collision", "strain_hardening", "w_garea", "ga_min", "ga_max")
 
 QUERY = {"perm": (1, np.int32), "mass": (2, np.float64), "system": (3, np.float64),
          "operator": (4, np.float64), "hinge_verts": (5, np.int32), "hinge_K": (6, np.float64),

@@ -145,6 +145,8 @@ int build_plan(int n, int T, const int32_t* tris, const double* X, const npfem_m
     return fail(NPFEM_EINVAL, "damping coefficients c_alpha, c_beta must be >= 0 (DESIGN.md A-20)");
   if (!(mat->strain_hardening >= 0.0))
     return fail(NPFEM_EINVAL, "strain_hardening must be >= 0 (DESIGN.md A-23)");
+  if (mat->w_garea != 0.0)
+    return fail(NPFEM_EINVAL, "the global-area term (w_garea != 0) exists in the oracle only (DESIGN.md A-24)");
   if (!(mat->w_collision >= 0.0) || !(mat->d_collision >= 0.0))
     return fail(NPFEM_EINVAL, "collision weight and contact distance must be >= 0 (DESIGN.md A-22)");
   if (!(mat->cell_mass > 0.0)) return fail(NPFEM_EINVAL, "cell_mass must be positive");

@@ -177,6 +177,16 @@ def test_operator_streams_hold_every_block_once_in_a_uniform_shape(cell):
     assert mma_needed <= mma_issued <= 1.6 * mma_needed + 12 * warps
 
 
+def test_global_area_term_is_rejected_by_the_cuda_library():
+    """The global-area term (reading A-24) exists in the oracle only: the product must say so
+    instead of silently ignoring the weight."""
+    rest, tris = W.rest_shape("rbc", 2)
+    with pytest.raises(NpfemError) as err:
+        NpfemPlan(tris, rest, W.default_material(rest, tris, w_garea=0.5), DT)
+    assert "oracle only" in str(err.value)
+    NpfemPlan(tris, rest, W.default_material(rest, tris, w_garea=0.0, ga_min=0.9, ga_max=1.1), DT)
+
+
 def test_global_mode_default_and_fallback():
     """Default = the fp16-split streams (3); a plan whose streams would need more than 64 slots per
     warp (here: the dense operator of RBC-3, 81 blocks in every row) falls back to 3xTF32 blocks (2),

@@ -793,3 +793,132 @@ def test_P26_strain_hardening_energy_force_and_fixed_point():
         xs, vs = c0.step_cell(xs, vs, pull, 10)
         xh, vh = c.step_cell(xh, vh, pull, 10)
     assert np.ptp(xh[:, 0]) < np.ptp(xs[:, 0]) - 1e-3
+
+
+# ----------------------------------------------------------------------------- global-area term (A-24)
+def test_P27_total_area_gradient_hessian_and_projection():
+    """Global-area term, geometry: (i) textbook areas (octahedron 4 sqrt 3, icosphere -> 4 pi from
+    below, translation invariance, scaling by s^2); (ii) grad A against central differences, with
+    sum_v grad_v A = 0 (translation) and sum_v x_v . grad_v A = 2 A (degree-2 homogeneity);
+    (iii) the Hessian against central differences of the gradient, symmetric, H x = grad A
+    (homogeneity again); (iv) the projection lands on A = A*, satisfies the KKT condition
+    P - x parallel to grad A(P), and is the closest such configuration: against SLSQP on the
+    perturbed tetrahedron / octahedron; (v) it converges where the volume's fixed-point iteration
+    does not (perturbed RBC-2 at a 12 % area excess)."""
+    assert O.area_total(OCT_T, OCT_V) == pytest.approx(4 * np.sqrt(3.0), rel=1e-14)
+    v, t = W.icosphere(3)
+    a = O.area_total(t, v)
+    assert 0.97 * 4 * np.pi < a < 4 * np.pi
+    assert O.area_total(t, v + np.array([50.0, -20.0, 7.0])) == pytest.approx(a, rel=1e-12)
+    assert O.area_total(t, 1.7 * v) == pytest.approx(1.7 ** 2 * a, rel=1e-13)
+    rng = np.random.default_rng(71)
+    x = OCT_V + 0.1 * rng.standard_normal(OCT_V.shape) + np.array([2.0, 1.0, -3.0])
+    g = O.area_grad(OCT_T, x)
+    H = O.area_hessian(OCT_T, x)
+    for i in range(6):
+        for d in range(3):
+            e = np.zeros_like(x); e[i, d] = 1e-6
+            fd = (O.area_total(OCT_T, x + e) - O.area_total(OCT_T, x - e)) / 2e-6
+            assert abs(fd - g[i, d]) < 1e-9
+            fdg = (O.area_grad(OCT_T, x + e) - O.area_grad(OCT_T, x - e)).ravel() / 2e-6
+            assert np.abs(fdg - H[:, 3 * i + d]).max() < 1e-8
+    assert np.allclose(g.sum(axis=0), 0, atol=1e-14)
+    xc = x - x.mean(axis=0)
+    assert np.sum(xc * g) == pytest.approx(2 * O.area_total(OCT_T, x), rel=1e-12)
+    assert np.abs(H - H.T).max() < 1e-14
+    assert np.abs(H @ x.ravel() - g.ravel()).max() < 1e-12               # grad A is degree-1 homogeneous
+    for verts, tris in ((TET_V, TET_T), (OCT_V, OCT_T)):
+        a0 = O.area_total(tris, verts)
+        for scale in (0.85, 1.05, 1.2):
+            x = verts * scale + 0.05 * rng.standard_normal(verts.shape) + np.array([3.0, -2.0, 1.0])
+            P, its = O.project_garea(tris, x, a0, a0)
+            assert 0 < its < 30
+            assert abs(O.area_total(tris, P) - a0) < 1e-13 * a0
+            gP, D = O.area_grad(tris, P).ravel(), (P - x).ravel()
+            assert np.abs(D - (D @ gP) / (gP @ gP) * gP).max() < 1e-12
+            cons = dict(type="eq", fun=lambda z: O.area_total(tris, z.reshape(-1, 3)) - a0,
+                        jac=lambda z: O.area_grad(tris, z.reshape(-1, 3)).ravel())
+            r = optimize.minimize(lambda z: 0.5 * np.sum((z - x.ravel()) ** 2), x.ravel(),
+                                  jac=lambda z: z - x.ravel(), constraints=[cons], method="SLSQP",
+                                  options=dict(ftol=1e-16, maxiter=500))
+            d_or, d_ref = np.linalg.norm(P - x), np.sqrt(2 * r.fun)
+            assert abs(d_or - d_ref) < 1e-7 * max(d_ref, 1e-3)
+            assert np.abs(P.ravel() - r.x).max() < 1e-6
+    rest, tris = W.rest_shape("rbc", 2)
+    x = rest * 1.06 + 0.02 * rng.standard_normal(rest.shape) + np.array([80.0, -30.0, 10.0])
+    a0 = O.area_total(tris, rest)
+    assert O.area_total(tris, x) > 1.1 * a0
+    P, its = O.project_garea(tris, x, a0, a0)
+    assert 0 < its < 15 and abs(O.area_total(tris, P) - a0) < 1e-12 * a0
+    gP, D = O.area_grad(tris, P).ravel(), (P - x).ravel()
+    assert np.abs(D - (D @ gP) / (gP @ gP) * gP).max() < 1e-12
+
+
+def test_P28_global_area_term_in_the_step():
+    """Global-area term in the solver (reading A-24): (i) closed form on the vertex-transitive
+    icosahedron scaled by s: the closest configuration with the rest area is the rest shape itself,
+    E = 1/2 w n R^2 (s-1)^2; (ii) w_garea sits on the diagonal of A_sys; (iii) f_int = -grad E by
+    central differences with the term on; (iv) the rest shape stays a fixed point; (v) the energy is
+    monotone over local/global half steps and the quasi-Newton identity (P-8) holds with the term;
+    (vi) the term does what it is for: under an inflating load the total area stays closer to A0;
+    (vii) weight 0 leaves everything bit-identical; negative weight and an inverted band are rejected."""
+    w = 0.8
+    v0, t0 = W.icosphere(0)
+    mat0 = W.default_material(v0, t0, w_garea=w, ga_min=1.0, ga_max=1.0)
+    ico = O.OracleCell(t0, v0, mat0, DT)
+    for sc in (0.9, 1.15):
+        P, e = ico.garea_local(sc * v0)
+        assert np.abs(P - v0).max() < 1e-12
+        assert e == pytest.approx(0.5 * w * 12 * (sc - 1) ** 2, rel=1e-12)
+    c, rest, tris, mat = make_cell("rbc", 2, w_garea=w, ga_min=1.0, ga_max=1.0)
+    c0, _, _, _ = make_cell("rbc", 2)
+    assert np.allclose(c.system_matrix() - c0.system_matrix(), w * np.eye(rest.shape[0]), atol=1e-12)
+    assert c.rest_area() == pytest.approx(O.area_total(tris, rest), rel=1e-13)
+    rng = np.random.default_rng(72)
+    x = rest * 1.06 + 0.02 * rng.standard_normal(rest.shape)
+    f = c.fint(x)
+
+    def E(y):
+        _, parts = c.energy(y, y, c.local(y), parts=True)
+        return parts[1:].sum() + c.garea_local(y)[1]
+
+    for _ in range(10):
+        i, d = rng.integers(rest.shape[0]), rng.integers(3)
+        e = np.zeros_like(x); e[i, d] = 1e-6
+        assert -(E(x + e) - E(x - e)) / 2e-6 == pytest.approx(f[i, d], rel=2e-5, abs=1e-9)
+    assert np.abs(f - c0.fint(x)).max() > 1e-3 * np.abs(f).max()
+    z = np.zeros_like(rest)
+    xr, vr = c.step_cell(rest, z, z, 10)
+    assert np.abs(xr - rest).max() < 1e-13
+    vel = 1e-3 * rng.standard_normal(rest.shape)
+    fext = 5e-3 * rng.standard_normal(rest.shape)
+    xs, vs, its, en = c.step_cell(x, vel, fext, 8, trace=True)
+    assert (np.diff(en) <= 1e-12 * np.abs(en[:-1])).all()
+    m = c.masses()[:, None]
+    s = x + DT * vel + DT * DT * fext / m
+    assert np.abs(its[0] - s).max() < 1e-15
+    grad = -c.fint(s)                                                     # x^0 = s: the inertia term vanishes
+    assert np.abs(its[1] - (s - np.linalg.solve(c.system_matrix(), grad))).max() < 1e-12
+    g_obj, g_grad = c.objective(x, s, x, grad=True)                       # converged-solve objective carries the term
+    for _ in range(4):
+        i, d = rng.integers(rest.shape[0]), rng.integers(3)
+        e = np.zeros_like(x); e[i, d] = 1e-6
+        fd = (c.objective(x + e, s, x) - c.objective(x - e, s, x)) / 2e-6
+        assert fd == pytest.approx(g_grad[i, d], rel=2e-5, abs=1e-8)
+    nrm = rest / np.linalg.norm(rest, axis=1, keepdims=True)
+    load = 2e-2 * nrm
+    xa, va, xb, vb = rest.copy(), z.copy(), rest.copy(), z.copy()
+    strong, _, _, _ = make_cell("rbc", 2, w_garea=20.0, ga_min=1.0, ga_max=1.0)
+    for _ in range(40):
+        xa, va = c0.step_cell(xa, va, load, 10)
+        xb, vb = strong.step_cell(xb, vb, load, 10)
+    a0 = c0.rest_area()
+    assert abs(O.area_total(tris, xb) - a0) < 0.7 * abs(O.area_total(tris, xa) - a0)
+    off, _, _, _ = make_cell("rbc", 2, w_garea=0.0, ga_min=1.0, ga_max=1.0)
+    pa, va2 = off.step_cell(x, vel, fext, 6)
+    pb, vb2 = c0.step_cell(x, vel, fext, 6)
+    assert np.array_equal(pa, pb) and np.array_equal(va2, vb2)
+    with pytest.raises(Exception):
+        make_cell("rbc", 2, w_garea=-1.0)
+    with pytest.raises(Exception):
+        make_cell("rbc", 2, w_garea=1.0, ga_min=1.2, ga_max=0.9)

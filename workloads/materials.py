@@ -29,6 +29,7 @@ def default_material(rest_xyz, tris, **overrides) -> dict:
         c_alpha=0.0, c_beta=0.0,
         w_collision=0.0, d_collision=0.0,
         strain_hardening=0.0,
+        w_garea=0.0, ga_min=1.0, ga_max=1.0,
     )
     for k, v in overrides.items():
         if k not in mat:
