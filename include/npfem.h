@@ -278,6 +278,11 @@ int npfem_plan_info(npfem_plan p, npfem_info* out);
                               /* descriptors, row table): every kept block exactly once                */
 #define NPFEM_Q_STREAM_SHAPE 14 /* int32 [10]: warps, slots per warp, three-product slots of row slots  */
                               /* 0..3, one-product slots of row slots 0..3                             */
+#define NPFEM_Q_STREAM_VAL 15  /* int32 [warps][slots][32 lanes][4]: the raw stream words (mma B         */
+                              /* fragments: fp16 pairs) exactly as the kernel loads them               */
+#define NPFEM_Q_STREAM_DESC 16 /* int32 [warps][32 lanes][4]: slot descriptors as the kernel loads them   */
+#define NPFEM_Q_STREAM_ROWS 17 /* int32 [4][32]: output block row of (row slot, warp), 255 = none         */
+#define NPFEM_Q_ROW_SCALE 18   /* double [n_verts]: 2^-k of each operator row's scaling, INTERNAL order   */
 int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems);
 
 #ifdef __cplusplus

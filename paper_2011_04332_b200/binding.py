@@ -21,7 +21,8 @@ QUERY = {"perm": (1, np.int32), "mass": (2, np.float64), "system": (3, np.float6
          "hinge_wr": (7, np.float64), "tri_dminv": (8, np.float64), "tri_area": (9, np.float64),
          "operator_x1": (10, np.float64), "operator_f16": (11, np.float64),
          "operator_f16x1": (12, np.float64), "operator_stream": (13, np.float64),
-         "stream_shape": (14, np.int32)}
+         "stream_shape": (14, np.int32), "stream_val": (15, np.int32), "stream_desc": (16, np.int32),
+         "stream_rows": (17, np.int32), "row_scale": (18, np.float64)}
 
 ERROR_NAMES = {0: "NPFEM_OK", -1: "NPFEM_EINVAL", -2: "NPFEM_ENOMEM", -3: "NPFEM_ECUDA",
                -4: "NPFEM_ELIMIT"}

@@ -239,6 +239,17 @@ int npfem_plan_query(npfem_plan p, int what, void* dst, int dst_elems) {
                            P.hs_nb[0], P.hs_nb[1], P.hs_nb[2], P.hs_nb[3]};
       return copy_out(shape, 10, sizeof(int32_t));
     }
+    case NPFEM_Q_STREAM_VAL: return copy_out(P.hs_val.data(), P.hs_val.size(), sizeof(uint32_t));
+    case NPFEM_Q_STREAM_DESC: return copy_out(P.hs_desc.data(), P.hs_desc.size(), sizeof(uint32_t));
+    case NPFEM_Q_STREAM_ROWS: {
+      int32_t rows[4 * 32];
+      for (int i = 0; i < 4 * 32; ++i) rows[i] = P.hs_rows[i];
+      return copy_out(rows, 4 * 32, sizeof(int32_t));
+    }
+    case NPFEM_Q_ROW_SCALE: {
+      std::vector<double> sc(P.hp_scale.begin(), P.hp_scale.end());
+      return copy_out(sc.data(), sc.size(), sizeof(double));
+    }
     case NPFEM_Q_OPERATOR_STREAM: {
       // walk the streams exactly as the kernel does: warp w, row slot j, first hs_na[j] three-product
       // slots (one pair: words 0,1 hi, 2,3 lo), then hs_nb[j] one-product slots (two pairs: hi, hi)

@@ -177,6 +177,109 @@ def test_operator_streams_hold_every_block_once_in_a_uniform_shape(cell):
     assert mma_needed <= mma_issued <= 1.6 * mma_needed + 12 * warps
 
 
+def _halves(words):
+    """uint32 words -> float64 pairs (low half = lower index), as fp16."""
+    w = np.asarray(words, dtype=np.uint32)
+    lo = (w & 0xffff).astype(np.uint16).view(np.float16).astype(np.float64)
+    hi = (w >> 16).astype(np.uint16).view(np.float16).astype(np.float64)
+    return lo, hi
+
+
+@pytest.mark.parametrize("kind,level", [("rbc", 2), ("plt", 1), ("rbc", 3)])
+def test_mode3_data_path_emulated_from_the_raw_streams(kind, level):
+    """The global_mode-3 product replayed on the CPU from the RAW arrays the kernel loads (stream
+    words, slot descriptors, row table, row scales), with the kernel's right-hand-side layout
+    (per source block a hi and a lo plane of 8-byte chunks {col g, col g+8} x vertices (2t, 2t+1),
+    chunk index (4 g + t) ^ 4 (kb & 7)) and the PTX fragment conventions of mma.m16n8k16 restated
+    here: A a0/a1 = rows g / g+8 at k = 2t, 2t+1, a2/a3 the same at k + 8; B b0 = k 2t, 2t+1 at
+    n = g, b1 = k + 8; D rows = right-hand-side columns, columns = output vertices.  The result
+    must be T r to fp32 accuracy: this pins the host side of the data path (streams, descriptors,
+    swizzle, scales) against those conventions without a GPU."""
+    rest, tris = W.rest_shape(kind, level)
+    mat = W.default_material(rest, tris)
+    plan = NpfemPlan(tris, rest, mat, DT)
+    n = rest.shape[0]
+    shape = plan.query("stream_shape")
+    warps, Q, na, nb = int(shape[0]), int(shape[1]), shape[2:6], shape[6:10]
+    val = plan.query("stream_val").view(np.uint32).reshape(warps, Q, 32, 4)
+    desc = plan.query("stream_desc").view(np.uint32).reshape(warps, 32, 4)
+    rows = plan.query("stream_rows").reshape(4, 32)
+    row_scale = plan.query("row_scale")
+    perm = plan.query("perm")
+    nvb = plan.info()["n_vblocks"]
+    NP = nvb * 8
+    rng = np.random.Generator(np.random.PCG64(23))
+    r = np.zeros((NP, 16), dtype=np.float32)                          # internal vertex order, 15 columns + pad
+    r[:n, :15] = (rng.standard_normal((n, 15)) * 10.0 ** rng.uniform(-4, 1, size=(1, 15))).astype(np.float32)
+    # split pass: per cell (3 columns) scale to max |r| in [2^13, 2^14), fp16 hi / lo, swizzled layout
+    buf = np.zeros(nvb * 512, dtype=np.uint8)
+    b16 = buf.view(np.uint16)
+    cell_exp = []
+    for c in range(5):
+        mx = np.abs(r[:, 3 * c:3 * c + 3]).max()
+        e = int(np.float32(mx).view(np.uint32) >> 23)                   # biased exponent, as the kernel takes it
+        e = min(max(e, 14), 254)
+        cell_exp.append(e)
+    for v in range(NP):
+        kb, k = v >> 3, v & 7
+        t, odd = k >> 1, k & 1
+        for m in range(16):
+            x = np.float32(r[v, m] * np.float32(2.0 ** (140 - cell_exp[m // 3]))) if m < 15 else np.float32(0)
+            hi = np.float16(x)
+            lo = np.float16(np.float32(x) - np.float32(hi))
+            g, up = m & 7, m >> 3
+            off = kb * 512 + (((g ^ (kb & 7)) * 4 + t) * 8) + up * 4 + odd * 2
+            b16[off // 2] = hi.view(np.uint16)
+            b16[(off + 256) // 2] = lo.view(np.uint16)
+    b32 = buf.view(np.uint32)
+
+    def afrag(off):                                                      # lane's 8 bytes at byte offset off: (a_even, a_odd)
+        return b32[off // 4], b32[off // 4 + 1]
+
+    dd = np.zeros((16, NP))
+    for w in range(warps):
+        q = 0
+        for j in range(4):
+            ib = int(rows[j, w])
+            D = np.zeros((16, 8))
+            for u in range(int(na[j] + nb[j])):
+                full = u < na[j]
+                for pr in range(1 if full else 2):
+                    dw = int(desc[w, q & 31, 2 * ((q >> 5) & 1) + pr])
+                    A_hi, A_lo = np.zeros((16, 16)), np.zeros((16, 16))
+                    B_hi, B_lo = np.zeros((16, 8)), np.zeros((16, 8))
+                    for lane in range(32):
+                        g, t = lane >> 2, lane & 3
+                        for half, o in enumerate(((dw & 0xffff) ^ (lane * 8), (dw >> 16) ^ (lane * 8))):
+                            for plane, A in ((0, A_hi), (256, A_lo)):
+                                w0, w1 = afrag(o + plane)
+                                (x0, x1), (y0, y1) = _halves(w0), _halves(w1)
+                                A[g, 2 * t + 8 * half], A[g, 2 * t + 1 + 8 * half] = x0, x1
+                                A[g + 8, 2 * t + 8 * half], A[g + 8, 2 * t + 1 + 8 * half] = y0, y1
+                        words = val[w, q, lane]
+                        bh = words[0:2] if full else words[2 * pr:2 * pr + 2]
+                        for half in range(2):
+                            x0, x1 = _halves(bh[half])
+                            B_hi[2 * t + 8 * half, g], B_hi[2 * t + 1 + 8 * half, g] = x0, x1
+                            if full:
+                                x0, x1 = _halves(words[2 + half])
+                                B_lo[2 * t + 8 * half, g], B_lo[2 * t + 1 + 8 * half, g] = x0, x1
+                    D += A_hi @ B_hi
+                    if full:
+                        D += A_lo @ B_hi + A_hi @ B_lo
+                q += 1
+            if ib != 255:
+                dd[:, ib * 8:ib * 8 + 8] = D
+    got = np.zeros((n, 15))
+    for v in range(n):
+        for m in range(15):
+            got[v, m] = dd[m, v] * row_scale[v] * 2.0 ** (cell_exp[m // 3] - 140)
+    op = plan.query("operator").reshape(n, n)[np.ix_(perm, perm)]    # internal order
+    want = op @ r[:n, :15].astype(np.float64)
+    bound = np.abs(op).sum(axis=1, keepdims=True) * np.abs(r[:n, :15]).reshape(n, 5, 3).max(axis=(0, 2)).repeat(3)[None, :]
+    assert (np.abs(got - want) <= 4 * 2.0 ** -24 * bound).all()
+
+
 def test_global_area_term_is_rejected_by_the_cuda_library():
     """The global-area term (reading A-24) exists in the oracle only: the product must say so
     instead of silently ignoring the weight."""
