@@ -447,6 +447,7 @@ def run_ours(args) -> None:
                        "smem_bytes": info["smem_bytes"], "global_mode": info["global_mode"],
                        "op_blocks": info["n_op_blocks"], "op_blocks_tf32x1": info["n_op_blocks_tf32x1"],
                        "op_blocks_f16x1": info["n_op_blocks_f16x1"],
+                       "ctas_per_sm": info["ctas_per_sm"], "tmem_columns": info["tmem_columns"],
                        "elements_per_cell": info["n_elements"],
                        "l2": "inputs (2.3 GB per step) exceed L2; no flush needed"},
             "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "clocks": clocks,

@@ -242,6 +242,12 @@ typedef struct {
   int n_diamonds;         /* edge (n_diamonds of them) plus triangles left single by the matching  */
   int n_op_blocks_f16x1;  /* global_mode 3: of n_op_blocks, blocks applied as ONE fp16 product (hi   */
                           /* parts only): their share of every row's l1 mass is <= 2^-13            */
+  int tmem_columns;       /* tensor-memory columns one CTA of the fixed-count step kernel allocates    */
+                          /* (64 per 4 warps, 80 with damping, rounded up to a power of two)          */
+  int ctas_per_sm;        /* resident CTAs per SM = min over shared memory (227 KB), tensor memory    */
+  int ctas_per_sm_limiter; /* (512 columns) and threads (2048); limiter: 1 shared memory, 2 tensor     */
+                          /* memory, 3 threads.  Small meshes (platelets) are limited by tensor       */
+                          /* memory, not by the shared memory the plan sizes                          */
   double rest_volume, total_mass, inv_drop_tol;
 } npfem_info;
 int npfem_get_info(npfem_handle h, npfem_info* out);

@@ -42,7 +42,8 @@ class Info(C.Structure):
     _fields_ = [(f, C.c_int) for f in (
         "n_verts", "n_tris", "n_hinges", "cell_stride", "cells_per_cta", "threads_per_cta",
         "smem_bytes", "n_vblocks", "n_op_blocks", "op_nnz", "global_mode",
-        "volume_inner_iters", "n_op_blocks_tf32x1", "n_elements", "n_diamonds", "n_op_blocks_f16x1")] + [(f, C.c_double) for f in ("rest_volume", "total_mass",
+        "volume_inner_iters", "n_op_blocks_tf32x1", "n_elements", "n_diamonds", "n_op_blocks_f16x1", "tmem_columns", "ctas_per_sm",
+        "ctas_per_sm_limiter")] + [(f, C.c_double) for f in ("rest_volume", "total_mass",
                                                             "inv_drop_tol")]
 
     def as_dict(self) -> dict:

@@ -58,6 +58,19 @@ void fill_info(const Plan& P, int cell_stride, npfem_info* o) {
   o->n_elements = P.E;
   o->n_diamonds = P.n_diamonds;
   o->n_op_blocks_f16x1 = P.n_op_blocks_h1;
+  {   // occupancy of the fixed-count step kernel (the same arithmetic as its tcgen05.alloc)
+    const int groups = (P.threads / 32 + 3) / 4;
+    int cols = 64;
+    while (cols < (P.damped ? 80 : 64) * groups) cols <<= 1;
+    o->tmem_columns = cols;
+    const int by_smem = (227 * 1024) / (P.smem_bytes + 1024);   // + static shared memory and the per-CTA reserve
+    const int by_tmem = 512 / cols, by_threads = 2048 / P.threads;
+    int best = by_smem, lim = 1;
+    if (by_tmem < best) { best = by_tmem; lim = 2; }
+    if (by_threads < best) { best = by_threads; lim = 3; }
+    o->ctas_per_sm = best < 1 ? 1 : best;
+    o->ctas_per_sm_limiter = lim;
+  }
   o->op_nnz = P.op_nnz;
   o->global_mode = P.global_mode;
   o->volume_inner_iters = P.opt.volume_inner_iters;

@@ -290,6 +290,19 @@ def test_global_area_term_is_rejected_by_the_cuda_library():
     NpfemPlan(tris, rest, W.default_material(rest, tris, w_garea=0.0, ga_min=0.9, ga_max=1.1), DT)
 
 
+def test_info_reports_the_occupancy_limiter():
+    """ADVICE (round 1): small meshes are limited by tensor-memory columns (64 per CTA, 512 per SM),
+    not by the shared memory the plan sizes; npfem_info says so.  RBC-3 fills one SM's shared memory."""
+    rest, tris = W.rest_shape("plt", 1)
+    info = NpfemPlan(tris, rest, W.default_material(rest, tris), DT).info()
+    assert info["tmem_columns"] == 64 and info["ctas_per_sm"] == 8 and info["ctas_per_sm_limiter"] == 2
+    rest, tris = W.rest_shape("rbc", 3)
+    info = NpfemPlan(tris, rest, W.default_material(rest, tris), DT).info()
+    assert info["tmem_columns"] == 512 and info["ctas_per_sm"] == 1 and info["ctas_per_sm_limiter"] == 1
+    damped = NpfemPlan(tris, rest, W.default_material(rest, tris, c_alpha=0.01), DT).info()
+    assert damped["tmem_columns"] == 512                                 # 6 groups x 80 columns
+
+
 def test_global_mode_default_and_fallback():
     """Default = the fp16-split streams (3); a plan whose streams would need more than 64 slots per
     warp (here: the dense operator of RBC-3, 81 blocks in every row) falls back to 3xTF32 blocks (2),
